@@ -1,0 +1,151 @@
+/*
+ * xy.h -- C-ABI boundary of the B200-native Swendsen-Wang sweep for the 2D classical XY model
+ * (arXiv 1210.6116, Komura & Okabe).  Plain pointers and sizes only; nothing throws or aborts
+ * across this boundary.  Every function returns XY_OK (0) or a negative XY_ERR_* code;
+ * xy_last_error() returns a thread-local, human-readable message for the last failure.
+ *
+ * The model (Eq. 3): H = -J sum_<ij> cos(theta_i - theta_j) on an L x L square
+ * lattice with periodic boundaries, J = 1.  Site index i = y*L + x (row-major);
+ * site i owns its +x bond to R(i) = y*L + (x+1 mod L) and its +y bond to D(i) = ((y+1) mod L)*L + x.
+ *
+ * One sweep (the hot path; Swendsen-Wang multi-cluster update PAPER.md:22 with Wolff's embedded
+ * cluster formalism PAPER.md:26; formulas as fixed in DESIGN.md section 3):
+ *   1. direction  phi_t uniform on [0, 2pi), r = (cos phi, sin phi)
+ *   2. projection sigma_i = s_i . r = cos(theta_i - phi)
+ *   3. bonds      bond <ij> active iff u < 1 - exp(-2 beta sigma_i sigma_j)   (decision in fp64)
+ *   4. labels     connected components of the active bonds; label = minimum site index
+ *   5. flip       each cluster reflected theta -> 2 phi + pi - theta (mod 2pi) with probability 1/2
+ *   6. observe    E, M, and the helicity-modulus link sums of Eq. 4-6
+ * All random numbers come from Philox4x32-10 keyed by (seed; index, sweep counter t, tag), so a
+ * sweep is a deterministic function of (theta, seed, t, beta).
+ *
+ * Threading / devices: a state is bound to the CUDA device current at creation and is not
+ * thread-safe.  "host" pointers are caller-owned host memory (pageable or pinned); "dev" pointers
+ * are caller-owned device memory.
+ */
+#ifndef XY_B200_H
+#define XY_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct xy_state xy_state;   /* opaque */
+
+enum { XY_INIT_COLD = 0,            /* all theta = +0.0f */
+       XY_INIT_HOT  = 1 };          /* theta_i = (float)(2pi * (w0>>8) * 2^-24), w = Philox(seed; i, 0, INIT) */
+
+enum { XY_OK = 0, XY_ERR_ARG = -1, XY_ERR_UNSUPPORTED_L = -2, XY_ERR_NOMEM = -3,
+       XY_ERR_CUDA = -4, XY_ERR_STATE = -5 };
+
+enum { XY_FLAG_LABELS64 = 1u };     /* hold labels as 64-bit words (default: 32-bit, enough for L <= 65536) */
+
+/* Observables of the configuration after `sweep` sweeps (PAPER.md:40 Eq. 3, :46-54 Eq. 4-6,
+ * :107 Eq. 9).  All sums are un-normalised and accumulated in fp64.
+ *   e_x = Cx/N, s_x = Sx/N,  Upsilon_x = <e_x> - beta N <s_x^2>,  <m^2> = <Mx^2+My^2>/N^2,  N = L^2. */
+typedef struct {
+    uint64_t sweep;                 /* T: number of sweeps done when this record was taken */
+    double   beta;                  /* beta of sweep T-1 (NaN for T = 0 or after xy_set_sweep) */
+    double   E, Mx, My;             /* E = -(Cx+Cy); Mx = sum cos theta_i; My = sum sin theta_i */
+    double   Cx, Sx, Cy, Sy;        /* sum cos / sin (theta_i - theta_R(i)) and (theta_i - theta_D(i)) */
+    uint64_t n_bonds_x, n_bonds_y, n_clusters;   /* of sweep T-1 (0 for T = 0) */
+} xy_obs;
+
+/* Schedule of the helicity-modulus PCC driver. */
+typedef struct {
+    uint64_t n_sweeps;              /* total sweeps of this call, including `discard` */
+    uint64_t discard;               /* sweeps at beta0 before the first window (paper: 60000) */
+    uint32_t window;                /* sweeps per beta*Upsilon estimate (paper: 1000); >= 1 */
+    uint32_t dirs;                  /* 1: x links only (paper); 2: mean of x and y links */
+    double   dbeta0;                /* informational copy of the initial step; the dbeta0 ARGUMENT wins */
+    uint64_t halve_every;           /* halve dbeta every this many measured sweeps; 0 = never (paper) */
+    double   dbeta_min;             /* floor for dbeta */
+    double   target;                /* critical beta*Upsilon: 0.636508 or 2/pi */
+} xy_pcc_schedule;
+
+typedef struct {
+    double   beta_final, dbeta_final;
+    double   beta_mean;             /* mean of beta over the decisions of the last dbeta stage that has any */
+    uint64_t n_decisions;
+    double  *trace_beta;            /* optional caller-allocated host arrays (may be NULL): beta the window ran at */
+    double  *trace_bY;              /*   and its beta*Upsilon estimate, one pair per decision */
+    uint64_t trace_cap;             /* capacity of the two arrays (entries) */
+    uint64_t trace_len;             /* out: number of decisions taken (may exceed trace_cap) */
+} xy_pcc_out;
+
+/* ---- the five calls of the problem statement ------------------------------------------------ */
+
+/* Create a state: L x L lattice, RNG seed, initial configuration XY_INIT_*; sweep counter t = 0.
+ * Device memory is allocated with cudaMalloc and owned by the state.  L must be a multiple of 64
+ * with 64 <= L <= 65536 (all sizes of PAPER.md:64), else XY_ERR_UNSUPPORTED_L. */
+int xy_create(xy_state **out, uint32_t L, uint64_t seed, int init);
+
+/* Run n Swendsen-Wang sweeps at inverse temperature beta (finite, >= 0).  Only ENQUEUES work on
+ * cuda_stream (a cudaStream_t passed as void*; NULL = the legacy default stream) and returns;
+ * the sweep counter advances by n.  xy_sw_sweeps(n) is identical to n calls of xy_sw_sweeps(1).
+ * XY_ERR_STATE if the counter would reach 2^32 (the RNG takes 32 bits of it). */
+int xy_sw_sweeps(xy_state *s, double beta, uint64_t n, void *cuda_stream);
+
+/* Observables of the current configuration (after all enqueued sweeps).  Synchronises the
+ * state's stream.  out: caller-owned host memory. */
+int xy_measure(xy_state *s, xy_obs *out);
+
+/* PCC run (raise beta by dbeta when beta*Upsilon < target, lower it otherwise), with
+ * the whole control loop on the device; blocking.  Starts at the state's current configuration and
+ * sweep counter, on the state's last-used stream.  Order of operations: DESIGN.md section 3 (O8). */
+int xy_pcc_run(xy_state *s, double beta0, double dbeta0, const xy_pcc_schedule *sched, xy_pcc_out *out);
+
+/* Free the state (and its device memory unless it was created on a caller workspace). */
+int xy_destroy(xy_state *s);
+
+/* ---- workspace-on-caller-memory variant (used by the PyTorch binding) ------------------------ */
+
+/* Bytes of device workspace a state of size L with `flags` needs. */
+int xy_workspace_bytes(uint32_t L, uint32_t flags, size_t *nbytes);
+
+/* As xy_create, with XY_FLAG_* flags, optionally on caller-owned DEVICE memory dev_workspace of
+ * nbytes >= xy_workspace_bytes (256-byte aligned; must outlive the state; xy_destroy then frees
+ * only host resources).  dev_workspace == NULL: allocate internally. */
+int xy_create_ex(xy_state **out, uint32_t L, uint64_t seed, int init, uint32_t flags,
+                 void *dev_workspace, size_t nbytes);
+
+/* ---- parity / checkpoint extensions (host buffers; each synchronises the state's stream) ----- */
+
+int xy_get_angles(xy_state *s, float *host, size_t n);          /* n must equal L*L */
+int xy_set_angles(xy_state *s, const float *host, size_t n);    /* values must lie in [0, 6.2831855] */
+/* canonical labels of the most recent sweep, label = minimum site index of the cluster, widened
+ * to int64 for every L; XY_ERR_STATE before the first sweep. */
+int xy_get_labels(xy_state *s, int64_t *host, size_t n);
+/* bonds of the most recent sweep, one byte per site: bit0 = x bond, bit1 = y bond. */
+int xy_get_bonds(xy_state *s, uint8_t *host, size_t n);
+/* per-sweep records for T = first_sweep .. first_sweep+count-1 from the device ring
+ * (capacity xy_series_capacity(); records older than that are gone -> XY_ERR_ARG). */
+int xy_get_series(xy_state *s, xy_obs *host, uint64_t first_sweep, uint64_t count);
+int xy_series_capacity(xy_state *s, uint64_t *cap);
+int xy_get_sweep(xy_state *s, uint64_t *t);
+int xy_set_sweep(xy_state *s, uint64_t t);                      /* resume / sampled-sweep parity */
+int xy_debug_fix_phi(xy_state *s, int on, double phi);          /* Ising-limit and 2x2-style tests */
+/* number of bond decisions of all sweeps so far that the fp32 filter could not settle and that
+ * were re-evaluated with the full fp64 expression. */
+int xy_get_fallback_count(xy_state *s, uint64_t *count);
+
+/* ---- step-level entry points for the parity tests -------------------------------------------- */
+
+/* Run only the labeling kernels (tile-local union-find, boundary merge) on an injected bond set
+ * (canonical byte layout as xy_get_bonds); read the result with xy_get_labels. */
+int xy_label_bonds(xy_state *s, const uint8_t *host_bonds, size_t n);
+/* Evaluate the CUDA path's own Philox4x32-10 device function on n (counter, key) pairs:
+ * ctr_host[4n], key_host[2n] -> out_host[4n]. */
+int xy_debug_philox(const uint32_t *ctr_host, const uint32_t *key_host, uint32_t *out_host, size_t n);
+/* Same inputs through NVIDIA cuRAND's curand_Philox4x32_10 device function (independent pin). */
+int xy_debug_curand_philox(const uint32_t *ctr_host, const uint32_t *key_host, uint32_t *out_host, size_t n);
+
+const char *xy_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* XY_B200_H */

@@ -1,0 +1,241 @@
+"""ctypes binding of include/xy.h: argument marshalling only (same names as the C calls).
+
+PyTorch is used for device memory (the workspace tensor handed to xy_create_ex), pinned host
+buffers and streams -- plumbing, not arithmetic.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libxy_b200.so")
+
+INIT_COLD, INIT_HOT = 0, 1
+FLAG_LABELS64 = 1
+
+
+class XYError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"xy error {code}: {msg}")
+        self.code = code
+
+
+def lib_path():
+    return _LIB_PATH
+
+
+def _load():
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(
+            f"{_LIB_PATH} is missing: build it with `python -m paper_1210_6116_b200.build` "
+            "(nvcc, sm_100a).  This package has no CPU fallback.")
+    return C.CDLL(_LIB_PATH)
+
+
+_lib = _load()
+
+
+class Obs(C.Structure):
+    _fields_ = [("sweep", C.c_uint64), ("beta", C.c_double),
+                ("E", C.c_double), ("Mx", C.c_double), ("My", C.c_double),
+                ("Cx", C.c_double), ("Sx", C.c_double), ("Cy", C.c_double), ("Sy", C.c_double),
+                ("n_bonds_x", C.c_uint64), ("n_bonds_y", C.c_uint64), ("n_clusters", C.c_uint64)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+OBS_DTYPE = np.dtype([("sweep", "<u8"), ("beta", "<f8"), ("E", "<f8"), ("Mx", "<f8"), ("My", "<f8"),
+                      ("Cx", "<f8"), ("Sx", "<f8"), ("Cy", "<f8"), ("Sy", "<f8"),
+                      ("n_bonds_x", "<u8"), ("n_bonds_y", "<u8"), ("n_clusters", "<u8")])
+assert OBS_DTYPE.itemsize == C.sizeof(Obs)
+
+
+class PccSchedule(C.Structure):
+    _fields_ = [("n_sweeps", C.c_uint64), ("discard", C.c_uint64),
+                ("window", C.c_uint32), ("dirs", C.c_uint32),
+                ("dbeta0", C.c_double), ("halve_every", C.c_uint64),
+                ("dbeta_min", C.c_double), ("target", C.c_double)]
+
+
+class _PccOut(C.Structure):
+    _fields_ = [("beta_final", C.c_double), ("dbeta_final", C.c_double), ("beta_mean", C.c_double),
+                ("n_decisions", C.c_uint64),
+                ("trace_beta", C.POINTER(C.c_double)), ("trace_bY", C.POINTER(C.c_double)),
+                ("trace_cap", C.c_uint64), ("trace_len", C.c_uint64)]
+
+
+_vp = C.c_void_p
+_SIGS = {
+    "xy_create": [C.POINTER(_vp), C.c_uint32, C.c_uint64, C.c_int],
+    "xy_create_ex": [C.POINTER(_vp), C.c_uint32, C.c_uint64, C.c_int, C.c_uint32, _vp, C.c_size_t],
+    "xy_workspace_bytes": [C.c_uint32, C.c_uint32, C.POINTER(C.c_size_t)],
+    "xy_sw_sweeps": [_vp, C.c_double, C.c_uint64, _vp],
+    "xy_measure": [_vp, C.POINTER(Obs)],
+    "xy_pcc_run": [_vp, C.c_double, C.c_double, C.POINTER(PccSchedule), C.POINTER(_PccOut)],
+    "xy_destroy": [_vp],
+    "xy_get_angles": [_vp, _vp, C.c_size_t],
+    "xy_set_angles": [_vp, _vp, C.c_size_t],
+    "xy_get_labels": [_vp, _vp, C.c_size_t],
+    "xy_get_bonds": [_vp, _vp, C.c_size_t],
+    "xy_get_series": [_vp, _vp, C.c_uint64, C.c_uint64],
+    "xy_series_capacity": [_vp, C.POINTER(C.c_uint64)],
+    "xy_get_sweep": [_vp, C.POINTER(C.c_uint64)],
+    "xy_set_sweep": [_vp, C.c_uint64],
+    "xy_debug_fix_phi": [_vp, C.c_int, C.c_double],
+    "xy_get_fallback_count": [_vp, C.POINTER(C.c_uint64)],
+    "xy_label_bonds": [_vp, _vp, C.c_size_t],
+    "xy_debug_philox": [_vp, _vp, _vp, C.c_size_t],
+    "xy_debug_curand_philox": [_vp, _vp, _vp, C.c_size_t],
+}
+for _name, _args in _SIGS.items():
+    _f = getattr(_lib, _name)
+    _f.argtypes = _args
+    _f.restype = C.c_int
+_lib.xy_last_error.restype = C.c_char_p
+_lib.xy_last_error.argtypes = []
+
+EXPORTED = tuple(_SIGS) + ("xy_last_error",)
+
+
+def _check(rc):
+    if rc != 0:
+        raise XYError(rc, _lib.xy_last_error().decode())
+
+
+def workspace_bytes(L, flags=0):
+    n = C.c_size_t()
+    _check(_lib.xy_workspace_bytes(L, flags, C.byref(n)))
+    return n.value
+
+
+def _host_ptr(arr):
+    """pointer of a contiguous numpy array or CPU torch tensor (pinned or pageable)."""
+    if isinstance(arr, np.ndarray):
+        assert arr.flags["C_CONTIGUOUS"]
+        return arr.ctypes.data
+    assert arr.device.type == "cpu" and arr.is_contiguous()
+    return arr.data_ptr()
+
+
+class XYState:
+    """One lattice on the current CUDA device.  Methods mirror the C calls one to one."""
+
+    def __init__(self, L, seed, init=INIT_HOT, flags=0, torch_workspace=True):
+        import torch
+        if not torch.cuda.is_available():
+            raise XYError(-4, "no CUDA device: this library has no CPU fallback")
+        self.L, self.N, self.seed, self.flags = L, L * L, seed, flags
+        self._h = _vp()
+        self._ws = None
+        if torch_workspace:
+            nbytes = workspace_bytes(L, flags)
+            self._ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+            _check(_lib.xy_create_ex(C.byref(self._h), L, seed, init, flags, self._ws.data_ptr(), nbytes))
+        else:
+            _check(_lib.xy_create_ex(C.byref(self._h), L, seed, init, flags, None, 0))
+
+    # -- the five calls ---------------------------------------------------------------------
+    def sw_sweeps(self, beta, n=1, stream=None):
+        import torch
+        st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+        _check(_lib.xy_sw_sweeps(self._h, beta, n, st))
+
+    def measure(self):
+        o = Obs()
+        _check(_lib.xy_measure(self._h, C.byref(o)))
+        return o
+
+    def pcc_run(self, beta0, sched: PccSchedule, trace=True):
+        out = _PccOut()
+        cap = int((sched.n_sweeps - sched.discard) // max(sched.window, 1)) if trace else 0
+        tb = np.zeros(max(cap, 1))
+        ty = np.zeros(max(cap, 1))
+        out.trace_beta = tb.ctypes.data_as(C.POINTER(C.c_double))
+        out.trace_bY = ty.ctypes.data_as(C.POINTER(C.c_double))
+        out.trace_cap = cap
+        _check(_lib.xy_pcc_run(self._h, beta0, sched.dbeta0, C.byref(sched), C.byref(out)))
+        n = min(int(out.trace_len), cap)
+        return {"beta_final": out.beta_final, "dbeta_final": out.dbeta_final, "beta_mean": out.beta_mean,
+                "n_decisions": int(out.n_decisions), "trace_len": int(out.trace_len),
+                "trace_beta": tb[:n].copy(), "trace_bY": ty[:n].copy()}
+
+    def destroy(self):
+        if self._h:
+            _check(_lib.xy_destroy(self._h))
+            self._h = _vp()
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    # -- extensions -------------------------------------------------------------------------
+    def get_angles(self, out=None):
+        out = np.empty(self.N, np.float32) if out is None else out
+        _check(_lib.xy_get_angles(self._h, _host_ptr(out), self.N))
+        return out
+
+    def set_angles(self, theta):
+        if isinstance(theta, np.ndarray):
+            theta = np.ascontiguousarray(theta, np.float32)
+        _check(_lib.xy_set_angles(self._h, _host_ptr(theta), self.N))
+
+    def get_labels(self):
+        out = np.empty(self.N, np.int64)
+        _check(_lib.xy_get_labels(self._h, out.ctypes.data, self.N))
+        return out
+
+    def get_bonds(self):
+        out = np.empty(self.N, np.uint8)
+        _check(_lib.xy_get_bonds(self._h, out.ctypes.data, self.N))
+        return out
+
+    def get_series(self, first, count):
+        out = np.zeros(count, OBS_DTYPE)
+        _check(_lib.xy_get_series(self._h, out.ctypes.data, first, count))
+        return out
+
+    def series_capacity(self):
+        c = C.c_uint64()
+        _check(_lib.xy_series_capacity(self._h, C.byref(c)))
+        return c.value
+
+    def get_sweep(self):
+        t = C.c_uint64()
+        _check(_lib.xy_get_sweep(self._h, C.byref(t)))
+        return t.value
+
+    def set_sweep(self, t):
+        _check(_lib.xy_set_sweep(self._h, t))
+
+    def debug_fix_phi(self, on, phi=0.0):
+        _check(_lib.xy_debug_fix_phi(self._h, 1 if on else 0, phi))
+
+    def get_fallback_count(self):
+        c = C.c_uint64()
+        _check(_lib.xy_get_fallback_count(self._h, C.byref(c)))
+        return c.value
+
+    def label_bonds(self, bonds):
+        b = np.ascontiguousarray(bonds, np.uint8)
+        _check(_lib.xy_label_bonds(self._h, b.ctypes.data, self.N))
+
+
+def _philox_common(fn, ctr, key):
+    ctr = np.ascontiguousarray(ctr, np.uint32).reshape(-1, 4)
+    key = np.ascontiguousarray(key, np.uint32).reshape(-1, 2)
+    out = np.zeros_like(ctr)
+    _check(fn(ctr.ctypes.data, key.ctypes.data, out.ctypes.data, ctr.shape[0]))
+    return out
+
+
+def debug_philox(ctr, key):
+    return _philox_common(_lib.xy_debug_philox, ctr, key)
+
+
+def debug_curand_philox(ctr, key):
+    return _philox_common(_lib.xy_debug_curand_philox, ctr, key)

@@ -1,0 +1,695 @@
+// xy_api.cu -- C-ABI boundary (include/xy.h) of the B200-native XY Swendsen-Wang sweep.
+// Host logic only: argument checks, workspace carving, per-sweep scalar parameters (direction
+// phi_t from the host-side Philox, the reflection constant), launch sequencing, ring bookkeeping.
+// Every step of the hot path runs in the kernels of xy_kernels.cuh; there is no CPU fallback.
+#include "xy_kernels.cuh"
+
+#include <curand_philox4x32_x.h>   // NVIDIA's curand_Philox4x32_10, for xy_debug_curand_philox only
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <limits>
+#include <new>
+
+using namespace xy;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                       \
+    do {                                                                                     \
+        cudaError_t e_ = (expr);                                                             \
+        if (e_ != cudaSuccess)                                                               \
+            return fail(e_ == cudaErrorMemoryAllocation ? XY_ERR_NOMEM : XY_ERR_CUDA,        \
+                        "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+constexpr uint32_t kRingCap = 16384;       // per-sweep records kept on the device
+constexpr uint32_t kMaxGrid = 148 * 16;    // upper bound for the persistent grids (partials array)
+constexpr size_t kStageBytes = 64u << 20;  // staging buffer of the debug getters
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Layout {
+    size_t theta, labels, bonds, partials, ring, ctl, total;
+};
+
+Layout make_layout(uint32_t L, uint32_t flags)
+{
+    const size_t N = (size_t)L * L;
+    const size_t lw = (flags & XY_FLAG_LABELS64) ? 8 : 4;
+    Layout o;
+    size_t off = 0;
+    o.theta = off;    off = align_up(off + N * 4, 256);
+    o.labels = off;   off = align_up(off + N * lw, 256);
+    o.bonds = off;    off = align_up(off + N / 4, 256);
+    o.partials = off; off = align_up(off + (size_t)kMaxGrid * kPartialStride * 8, 256);
+    o.ring = off;     off = align_up(off + (size_t)kRingCap * sizeof(xy_obs), 256);
+    o.ctl = off;      off = align_up(off + sizeof(DevCtl), 256);
+    o.total = off;
+    return o;
+}
+
+// One set of launchers per (tile geometry, label width).
+struct Kernels {
+    void (*bonds_label)(const SweepArgs &, int mode, int grid, cudaStream_t);
+    void (*merge)(const SweepArgs &, cudaStream_t);
+    void (*flip)(const SweepArgs &, int grid, cudaStream_t);
+    int (*occupancy)(int *bl_sweep, int *bl_obs, int *bl_label, int *fl);
+    int tw, th, threads;
+};
+
+template <int VEC, int R, int NW, typename LabelT>
+struct KS {
+    static void bonds_label(const SweepArgs &a, int mode, int grid, cudaStream_t st)
+    {
+        if (mode == MODE_SWEEP) k_bonds_label<VEC, R, NW, LabelT, MODE_SWEEP><<<grid, NW * 32, 0, st>>>(a);
+        else if (mode == MODE_OBS_ONLY) k_bonds_label<VEC, R, NW, LabelT, MODE_OBS_ONLY><<<grid, NW * 32, 0, st>>>(a);
+        else k_bonds_label<VEC, R, NW, LabelT, MODE_LABEL_ONLY><<<grid, NW * 32, 0, st>>>(a);
+    }
+    static void merge(const SweepArgs &a, cudaStream_t st)
+    {
+        const uint64_t total = (uint64_t)a.ntiles * (32 * VEC + R * NW);
+        uint64_t blocks = (total + 255) / 256;
+        if (blocks > 148ull * 64) blocks = 148ull * 64;
+        k_merge<32 * VEC, R * NW, LabelT><<<(unsigned)blocks, 256, 0, st>>>(a);
+    }
+    static void flip(const SweepArgs &a, int grid, cudaStream_t st)
+    {
+        k_flip<VEC, R, NW, LabelT><<<grid, NW * 32, 0, st>>>(a);
+    }
+    static int occupancy(int *bl_sweep, int *bl_obs, int *bl_label, int *fl)
+    {
+        cudaError_t e;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bl_sweep, k_bonds_label<VEC, R, NW, LabelT, MODE_SWEEP>, NW * 32, 0);
+        if (e != cudaSuccess) return (int)e;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bl_obs, k_bonds_label<VEC, R, NW, LabelT, MODE_OBS_ONLY>, NW * 32, 0);
+        if (e != cudaSuccess) return (int)e;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bl_label, k_bonds_label<VEC, R, NW, LabelT, MODE_LABEL_ONLY>, NW * 32, 0);
+        if (e != cudaSuccess) return (int)e;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(fl, k_flip<VEC, R, NW, LabelT>, NW * 32, 0);
+        return (int)e;
+    }
+    static Kernels get()
+    {
+        return Kernels{&bonds_label, &merge, &flip, &occupancy, 32 * VEC, R * NW, NW * 32};
+    }
+};
+
+constexpr int kR = 8, kNW = 8;   // 8 warps x 8 rows: tiles of 128 x 64 (VEC 4) or 64 x 64 (VEC 2)
+
+Kernels pick_kernels(uint32_t L, bool l64)
+{
+    if (L % 128 == 0) return l64 ? KS<4, kR, kNW, uint64_t>::get() : KS<4, kR, kNW, uint32_t>::get();
+    return l64 ? KS<2, kR, kNW, uint64_t>::get() : KS<2, kR, kNW, uint32_t>::get();
+}
+
+__global__ void k_debug_curand_philox(const uint32_t *ctr, const uint32_t *key, uint32_t *out, size_t n)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint4 c = make_uint4(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3]);
+    const uint2 k = make_uint2(key[2 * i], key[2 * i + 1]);
+    const uint4 w = curand_Philox4x32_10(c, k);
+    out[4 * i] = w.x; out[4 * i + 1] = w.y; out[4 * i + 2] = w.z; out[4 * i + 3] = w.w;
+}
+
+__global__ void k_ctl_init(DevCtl *c, xy_obs *ring, uint32_t ring_cap, uint64_t T)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        memset(c, 0, sizeof(DevCtl));
+        xy_obs *o = ring + (T % ring_cap);
+        memset(o, 0, sizeof(xy_obs));
+        o->sweep = T;
+        const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+        o->beta = qnan;
+        o->E = qnan; o->Mx = qnan; o->My = qnan; o->Cx = qnan; o->Sx = qnan; o->Cy = qnan; o->Sy = qnan;
+    }
+}
+
+__global__ void k_ring_reset(xy_obs *ring, uint32_t ring_cap, uint64_t T)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        xy_obs *o = ring + (T % ring_cap);
+        memset(o, 0, sizeof(xy_obs));
+        o->sweep = T;
+        const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+        o->beta = qnan;
+        o->E = qnan; o->Mx = qnan; o->My = qnan; o->Cx = qnan; o->Sx = qnan; o->Cy = qnan; o->Sy = qnan;
+    }
+}
+
+__global__ void k_check_angles(const float *theta, uint64_t N, unsigned int *flag)
+{
+    bool bad = false;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (uint64_t)gridDim.x * blockDim.x) {
+        const float v = theta[i];
+        bad |= !(v >= 0.0f && v <= 6.2831855f);
+    }
+    if (bad) atomicOr(flag, 1u);
+}
+
+struct PccSetup {
+    double beta0, dbeta0;
+    unsigned long long halve_every;
+    double dbeta_min, target;
+    unsigned int window, dirs;
+    double *trace_beta, *trace_bY;
+    unsigned long long trace_cap;
+};
+
+__global__ void k_pcc_setup(DevCtl *c, PccSetup s)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        c->beta = s.beta0; c->dbeta = s.dbeta0;
+        c->acc_e = 0; c->acc_s2 = 0; c->k = 0; c->n_dec = 0;
+        c->stage_sum = 0; c->last_sum = 0; c->stage_cnt = 0; c->last_cnt = 0;
+        c->halve_every = s.halve_every; c->dbeta_min = s.dbeta_min; c->target = s.target;
+        c->window = s.window; c->dirs = s.dirs;
+        c->trace_beta = s.trace_beta; c->trace_bY = s.trace_bY; c->trace_cap = s.trace_cap;
+    }
+}
+
+}  // namespace
+
+struct xy_state {
+    uint32_t L = 0, flags = 0;
+    uint64_t N = 0, seed = 0;
+    uint64_t T = 0;                 // sweeps done
+    int device = 0;
+    bool owns_ws = false;
+    char *ws = nullptr;
+    Layout lay{};
+    Kernels ker{};
+    int grid_bl = 0, grid_fl = 0;
+    cudaStream_t stream = nullptr;
+    bool have_sweep = false;        // bonds / labels of a sweep exist
+    bool labels_flat = false;
+    uint64_t obs_valid_T = UINT64_MAX;   // ring record whose observables are (or will be, in stream order) filled
+    uint64_t oldest_T = 0;          // oldest record still meaningful in the ring
+    bool fix_phi = false;
+    double phi_fixed = 0.0;
+    void *stage = nullptr;          // lazily allocated device staging for the getters
+
+    float *theta() const { return reinterpret_cast<float *>(ws + lay.theta); }
+    void *labels() const { return ws + lay.labels; }
+    uint8_t *bonds() const { return reinterpret_cast<uint8_t *>(ws + lay.bonds); }
+    double *partials() const { return reinterpret_cast<double *>(ws + lay.partials); }
+    xy_obs *ring() const { return reinterpret_cast<xy_obs *>(ws + lay.ring); }
+    DevCtl *ctl() const { return reinterpret_cast<DevCtl *>(ws + lay.ctl); }
+    bool l64() const { return (flags & XY_FLAG_LABELS64) != 0; }
+};
+
+namespace {
+
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+int check_L(uint32_t L)
+{
+    if (L < 64 || L > 65536 || (L % 64) != 0)
+        return fail(XY_ERR_UNSUPPORTED_L, "L=%u unsupported: need a multiple of 64 in [64, 65536]", L);
+    return XY_OK;
+}
+
+SweepArgs base_args(const xy_state *s)
+{
+    SweepArgs a;
+    memset(&a, 0, sizeof a);
+    a.theta = s->theta();
+    a.labels = s->labels();
+    a.bonds = s->bonds();
+    a.partials = s->partials();
+    a.ctl = s->ctl();
+    a.ring = s->ring();
+    a.ring_cap = kRingCap;
+    a.L = s->L;
+    a.tiles_x = s->L / s->ker.tw;
+    a.ntiles = a.tiles_x * (s->L / s->ker.th);
+    a.seed_lo = (uint32_t)(s->seed & 0xffffffffu);
+    a.seed_hi = (uint32_t)(s->seed >> 32);
+    a.t = (uint32_t)s->T;
+    return a;
+}
+
+// direction of sweep t and the constants derived from it (host side, once per sweep)
+void set_direction(const xy_state *s, uint64_t t, SweepArgs &a)
+{
+    double phi;
+    if (s->fix_phi) {
+        phi = s->phi_fixed;
+    } else {
+        const U4 w = rng((uint32_t)(s->seed & 0xffffffffu), (uint32_t)(s->seed >> 32), 0, (uint32_t)t, TAG_DIR);
+        phi = kTwoPi * ((double)w.x * (1.0 / 4294967296.0));
+    }
+    a.phi = phi;
+    a.cphi = std::cos(phi);
+    a.sphi = std::sin(phi);
+    volatile double A = 2.0 * phi;       // volatile: no contraction of the multiply-add on the host
+    A = A + kPi;
+    while (A >= kTwoPi) A = A - kTwoPi;
+    a.A = A;
+}
+
+int ensure_stage(xy_state *s)
+{
+    if (!s->stage) CUDA_TRY(cudaMalloc(&s->stage, kStageBytes));
+    return XY_OK;
+}
+
+// enqueue the observables of the current configuration (record T) if they are not on their way
+int ensure_obs(xy_state *s, int feed_pcc)
+{
+    if (s->obs_valid_T == s->T && !feed_pcc) return XY_OK;
+    SweepArgs a = base_args(s);
+    a.obs_fill = 1;
+    a.feed_pcc = feed_pcc;
+    s->ker.bonds_label(a, MODE_OBS_ONLY, s->grid_bl, s->stream);
+    CUDA_TRY(cudaGetLastError());
+    s->obs_valid_T = s->T;
+    return XY_OK;
+}
+
+// one sweep at the state's counter; beta_from_ctl: PCC mode
+int enqueue_sweep(xy_state *s, double beta, int beta_from_ctl, int feed_pcc)
+{
+    if (s->T >= 0xffffffffull) return fail(XY_ERR_STATE, "sweep counter would reach 2^32");
+    SweepArgs a = base_args(s);
+    set_direction(s, s->T, a);
+    a.beta = beta;
+    a.beta_from_ctl = beta_from_ctl;
+    a.feed_pcc = feed_pcc;
+    a.obs_fill = (s->obs_valid_T == s->T) ? 0 : 1;
+    s->ker.bonds_label(a, MODE_SWEEP, s->grid_bl, s->stream);
+    s->ker.merge(a, s->stream);
+    s->ker.flip(a, s->grid_fl, s->stream);
+    CUDA_TRY(cudaGetLastError());
+    if (a.obs_fill) s->obs_valid_T = s->T;
+    s->T += 1;
+    if (s->T - s->oldest_T >= kRingCap) s->oldest_T = s->T - kRingCap + 1;
+    s->have_sweep = true;
+    s->labels_flat = false;
+    return XY_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *xy_last_error(void) { return g_err; }
+
+int xy_workspace_bytes(uint32_t L, uint32_t flags, size_t *nbytes)
+{
+    if (!nbytes) return fail(XY_ERR_ARG, "nbytes is NULL");
+    if (int rc = check_L(L)) return rc;
+    if (flags & ~(uint32_t)XY_FLAG_LABELS64) return fail(XY_ERR_ARG, "unknown flags 0x%x", flags);
+    *nbytes = make_layout(L, flags).total;
+    return XY_OK;
+}
+
+int xy_create_ex(xy_state **out, uint32_t L, uint64_t seed, int init, uint32_t flags, void *dev_workspace, size_t nbytes)
+{
+    if (!out) return fail(XY_ERR_ARG, "out is NULL");
+    *out = nullptr;
+    if (int rc = check_L(L)) return rc;
+    if (init != XY_INIT_COLD && init != XY_INIT_HOT) return fail(XY_ERR_ARG, "init=%d unknown", init);
+    if (flags & ~(uint32_t)XY_FLAG_LABELS64) return fail(XY_ERR_ARG, "unknown flags 0x%x", flags);
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+        return fail(XY_ERR_CUDA, "no CUDA device: this library has no CPU fallback");
+    xy_state *s = new (std::nothrow) xy_state;
+    if (!s) return fail(XY_ERR_NOMEM, "host allocation failed");
+    s->L = L; s->N = (uint64_t)L * L; s->seed = seed; s->flags = flags;
+    s->lay = make_layout(L, flags);
+    s->ker = pick_kernels(L, s->l64());
+    cudaGetDevice(&s->device);
+    if (dev_workspace) {
+        if (nbytes < s->lay.total || ((uintptr_t)dev_workspace & 255u)) {
+            delete s;
+            return fail(XY_ERR_ARG, "workspace too small (%zu < %zu) or not 256-byte aligned", nbytes, make_layout(L, flags).total);
+        }
+        s->ws = static_cast<char *>(dev_workspace);
+    } else {
+        void *p = nullptr;
+        cudaError_t e = cudaMalloc(&p, s->lay.total);
+        if (e != cudaSuccess) {
+            const size_t want = s->lay.total;
+            delete s;
+            cudaGetLastError();
+            return fail(XY_ERR_NOMEM, "cudaMalloc(%zu) failed: %s", want, cudaGetErrorString(e));
+        }
+        s->ws = static_cast<char *>(p);
+        s->owns_ws = true;
+    }
+    int bl = 0, bo = 0, blab = 0, fl = 0, sms = 0;
+    cudaError_t e = (cudaError_t)s->ker.occupancy(&bl, &bo, &blab, &fl);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device);
+    if (e != cudaSuccess || bl < 1 || bo < 1 || blab < 1 || fl < 1) {
+        if (s->owns_ws) cudaFree(s->ws);
+        delete s;
+        return fail(XY_ERR_CUDA, "kernel occupancy query failed: %s (was the library built for this GPU's sm_100a?)",
+                    cudaGetErrorString(e));
+    }
+    const uint32_t ntiles = (L / s->ker.tw) * (L / s->ker.th);
+    // the three modes of k_bonds_label share ONE grid so that their fixed-order sums agree bitwise
+    int per_sm = bl < bo ? bl : bo;
+    if (blab < per_sm) per_sm = blab;
+    long g = (long)sms * per_sm;
+    if (g > (long)ntiles) g = ntiles;
+    if (g > (long)kMaxGrid) g = kMaxGrid;
+    s->grid_bl = (int)g;
+    g = (long)sms * fl;
+    if (g > (long)ntiles) g = ntiles;
+    s->grid_fl = (int)g;
+
+    if (init == XY_INIT_COLD) {
+        e = cudaMemsetAsync(s->theta(), 0, s->N * 4, nullptr);
+    } else {
+        k_init_hot<<<148 * 8, 256>>>(s->theta(), s->N, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32));
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) {
+        k_ctl_init<<<1, 32>>>(s->ctl(), s->ring(), kRingCap, 0);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(nullptr);
+    if (e != cudaSuccess) {
+        if (s->owns_ws) cudaFree(s->ws);
+        delete s;
+        return fail(XY_ERR_CUDA, "initialisation failed: %s", cudaGetErrorString(e));
+    }
+    *out = s;
+    return XY_OK;
+}
+
+int xy_create(xy_state **out, uint32_t L, uint64_t seed, int init)
+{
+    return xy_create_ex(out, L, seed, init, 0, nullptr, 0);
+}
+
+int xy_destroy(xy_state *s)
+{
+    if (!s) return XY_OK;
+    DeviceGuard g(s->device);
+    cudaStreamSynchronize(s->stream);
+    if (s->stage) cudaFree(s->stage);
+    if (s->owns_ws) cudaFree(s->ws);
+    delete s;
+    return XY_OK;
+}
+
+int xy_sw_sweeps(xy_state *s, double beta, uint64_t n, void *cuda_stream)
+{
+    if (!s) return fail(XY_ERR_ARG, "state is NULL");
+    if (!(beta >= 0.0) || !std::isfinite(beta)) return fail(XY_ERR_ARG, "beta must be finite and >= 0");
+    if (s->T + n > 0xffffffffull) return fail(XY_ERR_STATE, "sweep counter would reach 2^32");
+    DeviceGuard g(s->device);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (st != s->stream) {
+        // keep stream order across a change of stream
+        CUDA_TRY(cudaStreamSynchronize(s->stream));
+        s->stream = st;
+    }
+    for (uint64_t k = 0; k < n; ++k)
+        if (int rc = enqueue_sweep(s, beta, 0, 0)) return rc;
+    return XY_OK;
+}
+
+int xy_measure(xy_state *s, xy_obs *out)
+{
+    if (!s || !out) return fail(XY_ERR_ARG, "NULL argument");
+    DeviceGuard g(s->device);
+    if (int rc = ensure_obs(s, 0)) return rc;
+    CUDA_TRY(cudaMemcpyAsync(out, s->ring() + (s->T % kRingCap), sizeof(xy_obs), cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    return XY_OK;
+}
+
+int xy_pcc_run(xy_state *s, double beta0, double dbeta0, const xy_pcc_schedule *sc, xy_pcc_out *out)
+{
+    if (!s || !sc || !out) return fail(XY_ERR_ARG, "NULL argument");
+    if (!(beta0 >= 0.0) || !std::isfinite(beta0) || !(dbeta0 >= 0.0) || !std::isfinite(dbeta0))
+        return fail(XY_ERR_ARG, "beta0 and dbeta0 must be finite and >= 0");
+    if (sc->window < 1 || (sc->dirs != 1 && sc->dirs != 2)) return fail(XY_ERR_ARG, "window must be >= 1 and dirs 1 or 2");
+    if (sc->discard > sc->n_sweeps) return fail(XY_ERR_ARG, "discard > n_sweeps");
+    if (s->T + sc->n_sweeps > 0xffffffffull) return fail(XY_ERR_STATE, "sweep counter would reach 2^32");
+    DeviceGuard g(s->device);
+    const uint64_t measured = sc->n_sweeps - sc->discard;
+    const uint64_t max_dec = measured / sc->window;
+    double *d_trace = nullptr;
+    if (max_dec > 0) CUDA_TRY(cudaMalloc(&d_trace, max_dec * 2 * sizeof(double)));
+    PccSetup ps;
+    ps.beta0 = beta0; ps.dbeta0 = dbeta0;
+    ps.halve_every = sc->halve_every; ps.dbeta_min = sc->dbeta_min; ps.target = sc->target;
+    ps.window = sc->window; ps.dirs = sc->dirs;
+    ps.trace_beta = d_trace; ps.trace_bY = d_trace ? d_trace + max_dec : nullptr; ps.trace_cap = max_dec;
+    k_pcc_setup<<<1, 32, 0, s->stream>>>(s->ctl(), ps);
+    int rc = XY_OK;
+    bool feed_next = false;        // the next k_bonds_label feeds the record of the incoming state
+    for (uint64_t n = 0; n < sc->n_sweeps && rc == XY_OK; ++n) {
+        rc = enqueue_sweep(s, beta0, 1, feed_next ? 1 : 0);
+        feed_next = false;
+        if (rc != XY_OK || n < sc->discard) continue;
+        const uint64_t k = n - sc->discard + 1;
+        const bool decision = (k % sc->window) == 0;
+        if (decision || n + 1 == sc->n_sweeps) rc = ensure_obs(s, 1);   // beta must move before the next sweep reads it
+        else feed_next = true;
+    }
+    DevCtl h;
+    if (rc == XY_OK) {
+        cudaError_t e = cudaMemcpyAsync(&h, s->ctl(), sizeof h, cudaMemcpyDeviceToHost, s->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+        if (e == cudaSuccess && d_trace && out->trace_beta && out->trace_bY && out->trace_cap) {
+            const uint64_t ncopy = h.n_dec < out->trace_cap ? h.n_dec : out->trace_cap;
+            e = cudaMemcpy(out->trace_beta, d_trace, ncopy * sizeof(double), cudaMemcpyDeviceToHost);
+            if (e == cudaSuccess) e = cudaMemcpy(out->trace_bY, d_trace + max_dec, ncopy * sizeof(double), cudaMemcpyDeviceToHost);
+        }
+        if (e != cudaSuccess) rc = fail(XY_ERR_CUDA, "PCC run failed: %s", cudaGetErrorString(e));
+    } else {
+        cudaStreamSynchronize(s->stream);
+    }
+    if (d_trace) cudaFree(d_trace);
+    if (rc != XY_OK) return rc;
+    out->beta_final = h.beta;
+    out->dbeta_final = h.dbeta;
+    out->n_decisions = h.n_dec;
+    out->trace_len = h.n_dec;
+    if (h.stage_cnt > 0) out->beta_mean = h.stage_sum / (double)h.stage_cnt;
+    else if (h.last_cnt > 0) out->beta_mean = h.last_sum / (double)h.last_cnt;
+    else out->beta_mean = h.beta;
+    return XY_OK;
+}
+
+int xy_get_angles(xy_state *s, float *host, size_t n)
+{
+    if (!s || !host) return fail(XY_ERR_ARG, "NULL argument");
+    if (n != s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
+    DeviceGuard g(s->device);
+    CUDA_TRY(cudaMemcpyAsync(host, s->theta(), n * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    return XY_OK;
+}
+
+int xy_set_angles(xy_state *s, const float *host, size_t n)
+{
+    if (!s || !host) return fail(XY_ERR_ARG, "NULL argument");
+    if (n != s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
+    DeviceGuard g(s->device);
+    CUDA_TRY(cudaMemcpyAsync(s->theta(), host, n * sizeof(float), cudaMemcpyHostToDevice, s->stream));
+    k_ring_reset<<<1, 32, 0, s->stream>>>(s->ring(), kRingCap, s->T);
+    // range check on the device (the flag lives in the control block)
+    k_check_angles<<<148 * 8, 256, 0, s->stream>>>(s->theta(), s->N, &s->ctl()->pad);
+    unsigned int bad = 0;
+    CUDA_TRY(cudaMemcpyAsync(&bad, &s->ctl()->pad, sizeof bad, cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    s->obs_valid_T = UINT64_MAX;
+    s->oldest_T = s->T;
+    s->have_sweep = false;
+    if (bad) {
+        CUDA_TRY(cudaMemsetAsync(&s->ctl()->pad, 0, sizeof bad, s->stream));
+        return fail(XY_ERR_ARG, "angles outside [0, 6.2831855] (or NaN): the state now holds the rejected values");
+    }
+    return XY_OK;
+}
+
+int xy_get_sweep(xy_state *s, uint64_t *t)
+{
+    if (!s || !t) return fail(XY_ERR_ARG, "NULL argument");
+    *t = s->T;
+    return XY_OK;
+}
+
+int xy_set_sweep(xy_state *s, uint64_t t)
+{
+    if (!s) return fail(XY_ERR_ARG, "state is NULL");
+    if (t > 0xffffffffull) return fail(XY_ERR_STATE, "sweep counter must stay below 2^32");
+    DeviceGuard g(s->device);
+    s->T = t;
+    k_ring_reset<<<1, 32, 0, s->stream>>>(s->ring(), kRingCap, s->T);
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    s->obs_valid_T = UINT64_MAX;
+    s->oldest_T = t;
+    s->have_sweep = false;
+    return XY_OK;
+}
+
+int xy_debug_fix_phi(xy_state *s, int on, double phi)
+{
+    if (!s) return fail(XY_ERR_ARG, "state is NULL");
+    if (on && !std::isfinite(phi)) return fail(XY_ERR_ARG, "phi must be finite");
+    s->fix_phi = on != 0;
+    s->phi_fixed = phi;
+    return XY_OK;
+}
+
+int xy_series_capacity(xy_state *s, uint64_t *cap)
+{
+    if (!s || !cap) return fail(XY_ERR_ARG, "NULL argument");
+    *cap = kRingCap;
+    return XY_OK;
+}
+
+int xy_get_series(xy_state *s, xy_obs *host, uint64_t first, uint64_t count)
+{
+    if (!s || (!host && count)) return fail(XY_ERR_ARG, "NULL argument");
+    if (count == 0) return XY_OK;
+    if (first < s->oldest_T || first + count - 1 > s->T)
+        return fail(XY_ERR_ARG, "records %llu..%llu not in the ring (holds %llu..%llu)", (unsigned long long)first,
+                    (unsigned long long)(first + count - 1), (unsigned long long)s->oldest_T, (unsigned long long)s->T);
+    DeviceGuard g(s->device);
+    if (first + count - 1 == s->T)
+        if (int rc = ensure_obs(s, 0)) return rc;
+    uint64_t done = 0;
+    while (done < count) {
+        const uint64_t slot = (first + done) % kRingCap;
+        uint64_t run = kRingCap - slot;
+        if (run > count - done) run = count - done;
+        CUDA_TRY(cudaMemcpyAsync(host + done, s->ring() + slot, run * sizeof(xy_obs), cudaMemcpyDeviceToHost, s->stream));
+        done += run;
+    }
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    return XY_OK;
+}
+
+int xy_get_fallback_count(xy_state *s, uint64_t *count)
+{
+    if (!s || !count) return fail(XY_ERR_ARG, "NULL argument");
+    DeviceGuard g(s->device);
+    unsigned long long v = 0;
+    CUDA_TRY(cudaMemcpyAsync(&v, &s->ctl()->fallback_count, sizeof v, cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    *count = v;
+    return XY_OK;
+}
+
+int xy_get_labels(xy_state *s, int64_t *host, size_t n)
+{
+    if (!s || !host) return fail(XY_ERR_ARG, "NULL argument");
+    if (n != s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
+    if (!s->have_sweep) return fail(XY_ERR_STATE, "no sweep has produced labels yet");
+    DeviceGuard g(s->device);
+    if (int rc = ensure_stage(s)) return rc;
+    if (!s->labels_flat) {
+        if (s->l64()) k_flatten<uint64_t><<<148 * 8, 256, 0, s->stream>>>(static_cast<uint64_t *>(s->labels()), s->N);
+        else k_flatten<uint32_t><<<148 * 8, 256, 0, s->stream>>>(static_cast<uint32_t *>(s->labels()), s->N);
+        CUDA_TRY(cudaGetLastError());
+        s->labels_flat = true;
+    }
+    const uint64_t chunk = kStageBytes / sizeof(int64_t);
+    for (uint64_t first = 0; first < s->N; first += chunk) {
+        const uint64_t m = s->N - first < chunk ? s->N - first : chunk;
+        if (s->l64()) k_labels_to_i64<uint64_t><<<148 * 4, 256, 0, s->stream>>>(static_cast<const uint64_t *>(s->labels()), static_cast<int64_t *>(s->stage), first, m);
+        else k_labels_to_i64<uint32_t><<<148 * 4, 256, 0, s->stream>>>(static_cast<const uint32_t *>(s->labels()), static_cast<int64_t *>(s->stage), first, m);
+        CUDA_TRY(cudaMemcpyAsync(host + first, s->stage, m * sizeof(int64_t), cudaMemcpyDeviceToHost, s->stream));
+        CUDA_TRY(cudaStreamSynchronize(s->stream));
+    }
+    return XY_OK;
+}
+
+int xy_get_bonds(xy_state *s, uint8_t *host, size_t n)
+{
+    if (!s || !host) return fail(XY_ERR_ARG, "NULL argument");
+    if (n != s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
+    if (!s->have_sweep) return fail(XY_ERR_STATE, "no sweep has produced bonds yet");
+    DeviceGuard g(s->device);
+    if (int rc = ensure_stage(s)) return rc;
+    const uint64_t chunk = kStageBytes;
+    for (uint64_t first = 0; first < s->N; first += chunk) {
+        const uint64_t m = s->N - first < chunk ? s->N - first : chunk;
+        k_bonds_unpack<<<148 * 4, 256, 0, s->stream>>>(s->bonds(), static_cast<uint8_t *>(s->stage), first, m);
+        CUDA_TRY(cudaMemcpyAsync(host + first, s->stage, m, cudaMemcpyDeviceToHost, s->stream));
+        CUDA_TRY(cudaStreamSynchronize(s->stream));
+    }
+    return XY_OK;
+}
+
+int xy_label_bonds(xy_state *s, const uint8_t *host_bonds, size_t n)
+{
+    if (!s || !host_bonds) return fail(XY_ERR_ARG, "NULL argument");
+    if (n != s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
+    DeviceGuard g(s->device);
+    if (int rc = ensure_stage(s)) return rc;
+    const uint64_t chunk = kStageBytes;            // canonical bytes per pass (multiple of 4)
+    for (uint64_t first = 0; first < s->N; first += chunk) {
+        const uint64_t m = s->N - first < chunk ? s->N - first : chunk;
+        CUDA_TRY(cudaMemcpyAsync(s->stage, host_bonds + first, m, cudaMemcpyHostToDevice, s->stream));
+        k_bonds_pack<<<148 * 4, 256, 0, s->stream>>>(static_cast<const uint8_t *>(s->stage), s->bonds(), first / 4, m / 4);
+        CUDA_TRY(cudaStreamSynchronize(s->stream));
+    }
+    SweepArgs a = base_args(s);
+    s->ker.bonds_label(a, MODE_LABEL_ONLY, s->grid_bl, s->stream);
+    s->ker.merge(a, s->stream);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    s->have_sweep = true;
+    s->labels_flat = false;
+    return XY_OK;
+}
+
+static int debug_philox_common(const uint32_t *ctr, const uint32_t *key, uint32_t *out, size_t n, bool curand_fn)
+{
+    if (!ctr || !key || !out) return fail(XY_ERR_ARG, "NULL argument");
+    if (n == 0) return XY_OK;
+    uint32_t *d = nullptr;
+    CUDA_TRY(cudaMalloc(&d, n * 10 * sizeof(uint32_t)));
+    cudaError_t e = cudaMemcpy(d, ctr, n * 16, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(d + 4 * n, key, n * 8, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        const unsigned blocks = (unsigned)((n + 255) / 256);
+        if (curand_fn) k_debug_curand_philox<<<blocks, 256>>>(d, d + 4 * n, d + 6 * n, n);
+        else k_debug_philox<<<blocks, 256>>>(d, d + 4 * n, d + 6 * n, n);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(out, d + 6 * n, n * 16, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) return fail(XY_ERR_CUDA, "debug philox failed: %s", cudaGetErrorString(e));
+    return XY_OK;
+}
+
+int xy_debug_philox(const uint32_t *ctr, const uint32_t *key, uint32_t *out, size_t n)
+{
+    return debug_philox_common(ctr, key, out, n, false);
+}
+
+int xy_debug_curand_philox(const uint32_t *ctr, const uint32_t *key, uint32_t *out, size_t n)
+{
+    return debug_philox_common(ctr, key, out, n, true);
+}
+
+}  // extern "C"

@@ -1,0 +1,210 @@
+// xy_device.cuh -- device-side building blocks of the XY Swendsen-Wang sweep for sm_100a:
+// Philox4x32-10, fp64 sincos on [0, 2pi], the filtered bond decision, union-find helpers,
+// warp / block reductions.  Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace xy {
+
+constexpr double kTwoPi = 6.283185307179586;   // fl64(2 pi)
+constexpr double kPi    = 3.141592653589793;   // fl64(pi)
+
+enum : uint32_t { TAG_INIT = 0, TAG_DIR = 1, TAG_BOND = 2, TAG_FLIP = 3 };
+
+// ---------------------------------------------------------------------------------------------
+// Philox4x32 with 10 rounds (Salmon et al., SC'11).  Counter (c0..c3), key (k0,k1).
+// IMAD.WIDE.U32 gives hi and lo of each product in one instruction.
+// ---------------------------------------------------------------------------------------------
+struct U4 { uint32_t x, y, z, w; };
+
+__host__ __device__ __forceinline__ U4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                      uint32_t k0, uint32_t k1)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    return U4{c0, c1, c2, c3};
+}
+
+// counter = (idx lo, idx hi, (u32)t, tag); key = (seed lo, seed hi)
+__host__ __device__ __forceinline__ U4 rng(uint32_t seed_lo, uint32_t seed_hi, uint64_t idx, uint32_t t, uint32_t tag)
+{
+    return philox4x32_10((uint32_t)idx, (uint32_t)(idx >> 32), t, tag, seed_lo, seed_hi);
+}
+
+// ---------------------------------------------------------------------------------------------
+// sin and cos of an fp32 angle in [0, 2pi] (any |theta| < ~100 is fine), evaluated in fp64 with
+// |error| < 5e-13: Cody-Waite reduction by pi/2 in two pieces, Taylor polynomials on |r| <= pi/4
+// (sin through r^13: remainder (pi/4)^15/15! = 2e-14; cos through r^12: (pi/4)^14/14! = 4e-13).
+// This feeds the observables (tolerance 1e-9 per term) and the bond FILTER; bond decisions the
+// filter cannot settle are re-evaluated with libdevice cos/expm1 (bond_exact below).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void sincos_poly(float theta, double &s, double &c)
+{
+    const double t = (double)theta;
+    const double kd = __fma_rn(t, 0.6366197723675814, 6755399441055744.0);   // t * 2/pi, rounded to integer
+    const int q = __double2loint(kd);
+    const double k = kd - 6755399441055744.0;
+    double r = __fma_rn(-k, 1.5707963267948966, t);          // pi/2 high part
+    r = __fma_rn(-k, 6.123233995736766e-17, r);              // pi/2 low part
+    const double z = r * r;
+    double ps = -7.6471637318198164759e-13;                  // -1/15!
+    ps = __fma_rn(ps, z, 1.6059043836821614599e-10);         //  1/13!
+    ps = __fma_rn(ps, z, -2.5052108385441718775e-8);         // -1/11!
+    ps = __fma_rn(ps, z, 2.7557319223985890653e-6);          //  1/9!
+    ps = __fma_rn(ps, z, -1.9841269841269841270e-4);         // -1/7!
+    ps = __fma_rn(ps, z, 8.3333333333333333333e-3);          //  1/5!
+    ps = __fma_rn(ps, z, -1.6666666666666666667e-1);         // -1/3!
+    const double sr = __fma_rn(ps * z, r, r);
+    double pc = 2.0876756987868098979e-9;                    //  1/12!
+    pc = __fma_rn(pc, z, -2.7557319223985890653e-7);         // -1/10!
+    pc = __fma_rn(pc, z, 2.4801587301587301587e-5);          //  1/8!
+    pc = __fma_rn(pc, z, -1.3888888888888888889e-3);         // -1/6!
+    pc = __fma_rn(pc, z, 4.1666666666666666667e-2);          //  1/4!
+    pc = __fma_rn(pc, z, -0.5);
+    const double cr = __fma_rn(pc, z, 1.0);
+    // quadrant: q&1 swaps, q&2 negates sin, (q+1)&2 negates cos
+    const double a = (q & 1) ? cr : sr;
+    const double b = (q & 1) ? sr : cr;
+    s = (q & 2) ? -a : a;
+    c = ((q + 1) & 2) ? -b : b;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Bond decision.  Definition (fp64): active iff u < p, u = (w + 0.5) 2^-32,
+// p = -expm1(-2 beta sigma_i sigma_j), sigma = cos(theta - phi).
+// ---------------------------------------------------------------------------------------------
+__device__ __noinline__ bool bond_exact(float ti, float tj, double phi, double beta, uint32_t w,
+                                        unsigned long long *fallback_counter)
+{
+    const double si = cos(__dsub_rn((double)ti, phi));
+    const double sj = cos(__dsub_rn((double)tj, phi));
+    const double a = __dmul_rn(si, sj);
+    const double x = __dmul_rn(__dmul_rn(-2.0, beta), a);
+    const double p = -expm1(x);
+    const double u = __dmul_rn(__dadd_rn((double)w, 0.5), 1.0 / 4294967296.0);
+    atomicAdd(fallback_counter, 1ULL);
+    return u < p;
+}
+
+// Filter: e = 2^(a * m2b) with m2b = -2 beta log2(e) in fp32 approximates 1 - p; v = 1 - u.
+// |e32 - e| < 4e-7 for a >= 0 at ANY beta (the relative error of the exponent is bounded through
+// x 2^-x <= 0.531, the ex2.approx error is 2^-22 relative), |v32 - v| < 3.1e-8.  With delta = 2e-6
+// the sign of (e32 - v32) settles the decision whenever |e32 - v32| > delta; otherwise (2 delta of
+// all bonds) fall back to the exact fp64 expression.
+constexpr float kFilterDelta = 2e-6f;
+
+struct BondCtx {
+    double phi, beta;
+    float m2b;                                  // -2 beta log2(e), fp32
+    unsigned long long *fallback_counter;
+};
+
+__device__ __forceinline__ bool bond_decide(double a, uint32_t w, float ti, float tj, const BondCtx &cx)
+{
+    const float af = __double2float_rn(a);
+    float e;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(af * cx.m2b));
+    const float v = __uint2float_rn(~w) * 2.3283064365386963e-10f;   // (2^32-1-w) 2^-32 ~ 1-u
+    const float d = e - v;
+    if (fabsf(d) > kFilterDelta) return d < 0.0f;                    // e < 1-u  <=>  u < 1-e = p
+    return bond_exact(ti, tj, cx.phi, cx.beta, w, cx.fallback_counter);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Reflection theta -> 2 phi + pi - theta (mod 2pi), specified to the rounding: A is computed once
+// per sweep on the host (A = 2 phi + pi reduced into [0, 2pi)); here only add/sub/convert.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ float reflect(float theta, double A)
+{
+    double d = __dsub_rn(A, (double)theta);
+    while (d < 0.0) d = __dadd_rn(d, kTwoPi);
+    return __double2float_rn(d);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Union-find in shared memory (tile-local) and global memory (boundary merge).  Links always go
+// from the larger to the smaller index, so the root of a component is its minimum index.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t sfind(const volatile uint32_t *p, uint32_t a)
+{
+    uint32_t r = p[a];
+    while (r != a) { a = r; r = p[a]; }
+    return a;
+}
+
+__device__ __forceinline__ void sunion(uint32_t *p, uint32_t a, uint32_t b)
+{
+    for (;;) {
+        a = sfind(p, a);
+        b = sfind(p, b);
+        if (a == b) return;
+        if (a < b) { const uint32_t t = a; a = b; b = t; }      // a > b: link a -> b
+        const uint32_t old = atomicMin(&p[a], b);
+        if (old == a) return;
+        a = old;                                                 // a was re-linked meanwhile: carry on with its parent
+    }
+}
+
+template <typename T> struct AtomT;
+template <> struct AtomT<uint32_t> { using type = unsigned int; };
+template <> struct AtomT<uint64_t> { using type = unsigned long long; };
+
+template <typename LabelT>
+__device__ __forceinline__ LabelT gload(const LabelT *p)        // L2-coherent load (other SMs update concurrently)
+{
+    return __ldcg(p);
+}
+
+template <typename LabelT>
+__device__ __forceinline__ LabelT gfind(LabelT *lab, LabelT a)
+{
+    LabelT r = gload(lab + a);
+    while (r != a) { a = r; r = gload(lab + a); }
+    return a;
+}
+
+template <typename LabelT>
+__device__ __forceinline__ void gunion(LabelT *lab, LabelT a, LabelT b)
+{
+    using A = typename AtomT<LabelT>::type;
+    for (;;) {
+        a = gfind(lab, a);
+        b = gfind(lab, b);
+        if (a == b) return;
+        if (a < b) { const LabelT t = a; a = b; b = t; }
+        const LabelT old = (LabelT)atomicMin(reinterpret_cast<A *>(lab + a), (A)b);
+        if (old == a) return;
+        a = old;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Reductions with a fixed summation tree (bitwise reproducible for a fixed launch shape).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+}  // namespace xy
