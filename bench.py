@@ -1,0 +1,327 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Swendsen-Wang sweep of the 2D XY model (arXiv 1210.6116) on B200.
+
+    python bench.py --gpus N --steps K --warmup W [--workload cfg4] [--impl reference]
+
+A "step" is ONE whole sweep (projection + bond activation + cluster labeling + flip, with the
+observables of every sweep reduced on the device) of one lattice.  Metric: spin updates/s =
+L^2 * sweeps / time (BASELINE.json).  Default workload: BASELINE config 4 (L = 16384, beta = 1.11996,
+cold start, 500 thermalisation sweeps before anything is timed) -- the size the north_star's
+>= 60 % HBM target is stated for.  The path does not shard (clusters span the lattice): --gpus N
+runs N independent replicas (seed + rank), one process per GPU, no data-path collective.
+
+One JSON line on stdout (rank 0).  `value`: device-resident throughput; `e2e`: the same through the
+C-ABI with HOST buffers every step (xy_set_angles from pinned memory, one sweep, xy_get_angles +
+xy_measure back); `roofline`: dominant kernel, algorithmic bytes / CUDA-event time against the
+measured HBM copy bandwidth; `cpu_baseline`: the CPU oracle, as it stands, on a bounded sample.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import xy_inputs  # noqa: E402
+
+METRIC = "SW spin updates/s"
+UNIT = "spin updates/s"
+
+WORKLOADS = {
+    # name: (config index in BASELINE.json, L, init, seed, beta, thermalisation sweeps)
+    "cfg1": (0, 64, "hot", 1, 1.12, 0),
+    "cfg2": (1, 1024, "cold", 7, 1.12, 2000),
+    "cfg3": (2, 4096, "hot", 11, 1.11097, 200),      # fixed beta near the PCC run's end point
+    "cfg4": (3, 16384, "cold", 13, 1.11996, 500),
+    "cfg5": (4, 65536, "hot", 17, 1.11996, 0),
+    "L8192": (None, 8192, "cold", 13, 1.11996, 500),
+    "L32768": (None, 32768, "hot", 17, 1.11996, 50),
+}
+CPU_SAMPLE_L = 1024           # the oracle's bounded sample: a 1024^2 lattice of the same model
+
+
+def bytes_model(L, label_bytes, tw, th):
+    """Algorithmic (compulsory) DRAM bytes per site per launch of each kernel, DESIGN.md section 6."""
+    w = label_bytes
+    return {
+        "k_bonds": 4.0 + 0.25,                                  # theta read, packed bond bits written
+        "k_label": 0.25 + w,                                    # bond bits read, provisional label written
+        "k_merge": (tw + th) * (2.0 * w + 0.125) / (tw * th),   # two labels + the bond bit per tile-edge site
+        "k_flip": w + 4.0 + 4.0,                                # label read, theta read, theta written
+    }
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def cpu_oracle_rate(beta, budget_s=20.0, max_sweeps=None):
+    """the oracle as it stands, single thread, on a 1024^2 cold-start lattice; returns (rate, sweeps, secs)."""
+    from oracle import xy_oracle as xo
+    L = CPU_SAMPLE_L
+    th = xo.init(L, 13, xo.INIT_COLD)
+    t0 = time.perf_counter()
+    xo.run(th, L, 13, 0, beta, 1, series=True)
+    per = time.perf_counter() - t0
+    n = max(2, int(budget_s / max(per, 1e-3)))
+    if max_sweeps:
+        n = min(n, max_sweeps)
+    t0 = time.perf_counter()
+    xo.run(th, L, 13, 1, beta, n, series=True)
+    dt = time.perf_counter() - t0
+    return L * L * n / dt, n, dt
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the CPU oracle timed on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    from oracle import xy_oracle as xo
+    _, Lw, init, seed, beta, _ = WORKLOADS[args.workload]
+    L = CPU_SAMPLE_L
+    th = xo.init(L, seed, xo.INIT_COLD if init == "cold" else xo.INIT_HOT)
+    t = 0
+    for _ in range(args.warmup):
+        xo.run(th, L, seed, t, beta, 1, series=True)
+        t += 1
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        xo.run(th, L, seed, t, beta, 1, series=True)
+        t += 1
+    dt = time.perf_counter() - t0
+    val = L * L * args.steps / dt
+    sample = f"each step = one oracle sweep of a {L}x{L} lattice of the same model and beta (1/{(Lw // L) ** 2} of the workload's sites), single thread"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: L={Lw} beta={beta} {init} start (timed on the bounded sample)"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg4", choices=sorted(WORKLOADS))
+    ap.add_argument("--labels64", action="store_true", help="hold labels as 64-bit words")
+    ap.add_argument("--e2e-steps", type=int, default=None)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_1210_6116_b200 as xy
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    cfg_idx, L, init, seed, beta, therm = WORKLOADS[args.workload]
+    N = L * L
+    flags = xy.FLAG_LABELS64 if args.labels64 else 0
+    label_bytes = 8 if args.labels64 else 4
+    tw, th = (128, 64) if L % 128 == 0 else (64, 64)
+    K, W = args.steps, max(args.warmup, 0)
+
+    st = xy.XYState(L, seed + rank, xy_inputs.INIT_CODE[init], flags=flags)
+    if therm:
+        st.sw_sweeps(beta, therm)
+    st.sw_sweeps(beta, W)
+    torch.cuda.synchronize()
+
+    # ---- timed region 1: K sweeps, configuration resident in HBM ----
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    launches0 = st.get_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    st.sw_sweeps(beta, K)
+    e1.record()
+    barrier()
+    ms = max_over_ranks(e0.elapsed_time(e1))
+    launches = st.get_launch_count() - launches0
+    clocks = sampler.stop()
+    value = world * N * K / (ms * 1e-3)
+    obs = st.measure()
+
+    # ---- timed region 2: the same K sweeps with CUDA events around every kernel ----
+    st.debug_kernel_timing(True)
+    barrier()
+    st.sw_sweeps(beta, K)
+    kt = st.get_kernel_times()
+    st.debug_kernel_timing(False)
+    peak, peak_src = measured_peaks()
+    model = bytes_model(L, label_bytes, tw, th)
+    kern = {}
+    tot_ms = sum(v["ms"] for v in kt.values())
+    for name, v in kt.items():
+        avg = v["ms"] / max(v["launches"], 1)
+        gbs = model[name] * N / (avg * 1e-3) / 1e9 if avg > 0 else 0.0
+        kern[name] = {"avg_ms": avg, "share": v["ms"] / tot_ms if tot_ms else 0.0,
+                      "bytes_per_site": model[name], "achieved_gbs": gbs, "frac": gbs / peak}
+    dom = max(kern, key=lambda k: kern[k]["avg_ms"])
+    sweep_bytes = sum(model.values())
+    sweep_gbs = sweep_bytes * N * K / (ms * 1e-3) / 1e9
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(args.workload, {}).get(dom)
+        except Exception:
+            traffic = None
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["achieved_gbs"], "peak": peak,
+                "unit": "GB/s", "frac": kern[dom]["frac"], "traffic": traffic, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": model[dom] * N}
+
+    # ---- e2e: host buffers through the C-ABI every step ----
+    e2e = None
+    if not args.no_e2e:
+        ke = args.e2e_steps or max(3, min(K, 10))
+        host = torch.empty(N, dtype=torch.float32, pin_memory=True)
+        st.get_angles(host)
+        for _ in range(2):
+            st.set_angles(host); st.sw_sweeps(beta, 1); st.get_angles(host); st.measure()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(ke):
+            st.set_angles(host)          # H2D from pinned memory (synchronises)
+            st.sw_sweeps(beta, 1)
+            st.get_angles(host)          # D2H
+            st.measure()                 # D2H of the sweep's record
+        torch.cuda.synchronize()
+        dt = max_over_ranks(time.perf_counter() - t0)
+        e2e = {"value": world * N * ke / dt, "unit": UNIT, "h2d_bytes_per_step": N * 4,
+               "d2h_bytes_per_step": N * 4 + 104, "steps": ke, "ms_per_step": dt / ke * 1e3}
+        del host
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        rate, n, dt = cpu_oracle_rate(beta)
+        cpu = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"{n} oracle sweeps of a {CPU_SAMPLE_L}x{CPU_SAMPLE_L} cold-start lattice at beta={beta} "
+                         f"({dt:.1f} s, single thread; 1/{(L // CPU_SAMPLE_L) ** 2 if L >= CPU_SAMPLE_L else 1} of the workload's sites)"}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"BASELINE config {cfg_idx + 1 if cfg_idx is not None else '-'} ({args.workload}): "
+                                   f"2D XY L={L} periodic, {init} start seed {seed}, beta={beta}, "
+                                   f"{therm} thermalisation sweeps untimed",
+                       "L": L, "beta": beta, "label_bytes": label_bytes, "tile": f"{tw}x{th}",
+                       "replicas": world, "parallelism": "replicas only (the path does not shard)",
+                       "l2": "working set %.2f GiB per sweep >> 126 MB L2, no flush needed" % ((4 + label_bytes + 0.25) * N / 2 ** 30)
+                       if (4 + label_bytes) * N > 4 * 126e6 else "working set fits L2: number is NOT an HBM measurement"},
+            "clocks": clocks, "gpu_launches": int(launches),
+            "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
+            "kernels": kern,
+            "sweep_roofline": {"bytes_per_site": sweep_bytes, "achieved_gbs": sweep_gbs, "frac": sweep_gbs / peak,
+                               "floor_bytes_per_site": 8.0 + 2 * label_bytes,
+                               "ns_per_site": ms * 1e6 / (K * N)},
+            "observables": {"sweep": int(obs.sweep), "E_per_site": obs.E / N,
+                            "m2": (obs.Mx ** 2 + obs.My ** 2) / N ** 2,
+                            "bond_density": (obs.n_bonds_x + obs.n_bonds_y) / (2 * N),
+                            "clusters_per_site": obs.n_clusters / N},
+        }
+        print(json.dumps(line), flush=True)
+    st.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

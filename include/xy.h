@@ -132,6 +132,17 @@ int xy_debug_fix_phi(xy_state *s, int on, double phi);          /* Ising-limit a
  * were re-evaluated with the full fp64 expression. */
 int xy_get_fallback_count(xy_state *s, uint64_t *count);
 
+/* ---- measurement hooks (bench.py) ----------------------------------------------------------- */
+
+/* on != 0: record CUDA events on the state's stream around every kernel of every following sweep
+ * (k_bonds, k_label, k_merge, k_flip), so that per-kernel device time can be read back; off: stop. */
+int xy_debug_kernel_timing(xy_state *s, int on);
+/* Synchronise and return, accumulated since timing was switched on: device milliseconds and launch
+ * counts of [0] k_bonds, [1] k_label, [2] k_merge, [3] k_flip.  Resets the accumulators. */
+int xy_get_kernel_times(xy_state *s, double ms[4], uint64_t launches[4]);
+/* Total number of kernels this state has launched so far (all kinds). */
+int xy_get_launch_count(xy_state *s, uint64_t *count);
+
 /* ---- step-level entry points for the parity tests -------------------------------------------- */
 
 /* Run only the labeling kernels (tile-local union-find, boundary merge) on an injected bond set

@@ -85,6 +85,9 @@ _SIGS = {
     "xy_set_sweep": [_vp, C.c_uint64],
     "xy_debug_fix_phi": [_vp, C.c_int, C.c_double],
     "xy_get_fallback_count": [_vp, C.POINTER(C.c_uint64)],
+    "xy_debug_kernel_timing": [_vp, C.c_int],
+    "xy_get_kernel_times": [_vp, C.POINTER(C.c_double), C.POINTER(C.c_uint64)],
+    "xy_get_launch_count": [_vp, C.POINTER(C.c_uint64)],
     "xy_label_bonds": [_vp, _vp, C.c_size_t],
     "xy_debug_philox": [_vp, _vp, _vp, C.c_size_t],
     "xy_debug_curand_philox": [_vp, _vp, _vp, C.c_size_t],
@@ -218,6 +221,21 @@ class XYState:
     def get_fallback_count(self):
         c = C.c_uint64()
         _check(_lib.xy_get_fallback_count(self._h, C.byref(c)))
+        return c.value
+
+    def debug_kernel_timing(self, on):
+        _check(_lib.xy_debug_kernel_timing(self._h, 1 if on else 0))
+
+    def get_kernel_times(self):
+        ms = (C.c_double * 4)()
+        n = (C.c_uint64 * 4)()
+        _check(_lib.xy_get_kernel_times(self._h, ms, n))
+        names = ("k_bonds", "k_label", "k_merge", "k_flip")
+        return {k: {"ms": ms[i], "launches": int(n[i])} for i, k in enumerate(names)}
+
+    def get_launch_count(self):
+        c = C.c_uint64()
+        _check(_lib.xy_get_launch_count(self._h, C.byref(c)))
         return c.value
 
     def label_bonds(self, bonds):

@@ -13,6 +13,7 @@
 #include <cstring>
 #include <limits>
 #include <new>
+#include <vector>
 
 using namespace xy;
 
@@ -44,7 +45,7 @@ constexpr size_t kStageBytes = 64u << 20;  // staging buffer of the debug getter
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-    size_t theta, labels, bonds, partials, ring, ctl, total;
+    size_t theta, labels, bonds, partials, ring, ctl, tab, total;
 };
 
 Layout make_layout(uint32_t L, uint32_t flags)
@@ -59,26 +60,34 @@ Layout make_layout(uint32_t L, uint32_t flags)
     o.partials = off; off = align_up(off + (size_t)kMaxGrid * kPartialStride * 8, 256);
     o.ring = off;     off = align_up(off + (size_t)kRingCap * sizeof(xy_obs), 256);
     o.ctl = off;      off = align_up(off + sizeof(DevCtl), 256);
+    o.tab = off;      off = align_up(off + (size_t)(kTabN + 1) * sizeof(double2), 256);
     o.total = off;
     return o;
 }
 
 // One set of launchers per (tile geometry, label width).
 struct Kernels {
-    void (*bonds_label)(const SweepArgs &, int mode, int grid, cudaStream_t);
+    void (*bonds)(const SweepArgs &, bool obs_only, int grid, cudaStream_t);
+    void (*label)(const SweepArgs &, cudaStream_t);
     void (*merge)(const SweepArgs &, cudaStream_t);
     void (*flip)(const SweepArgs &, int grid, cudaStream_t);
-    int (*occupancy)(int *bl_sweep, int *bl_obs, int *bl_label, int *fl);
-    int tw, th, threads;
+    int (*occupancy)(int *bonds_sweep, int *bonds_obs, int *fl);
+    int tw, th, rs;
 };
+
+constexpr int kRS = 32;          // rows per warp strip in k_bonds
+constexpr int kBondsWarps = 4;   // warps per CTA in k_bonds
 
 template <int VEC, int R, int NW, typename LabelT>
 struct KS {
-    static void bonds_label(const SweepArgs &a, int mode, int grid, cudaStream_t st)
+    static void bonds(const SweepArgs &a, bool obs_only, int grid, cudaStream_t st)
     {
-        if (mode == MODE_SWEEP) k_bonds_label<VEC, R, NW, LabelT, MODE_SWEEP><<<grid, NW * 32, 0, st>>>(a);
-        else if (mode == MODE_OBS_ONLY) k_bonds_label<VEC, R, NW, LabelT, MODE_OBS_ONLY><<<grid, NW * 32, 0, st>>>(a);
-        else k_bonds_label<VEC, R, NW, LabelT, MODE_LABEL_ONLY><<<grid, NW * 32, 0, st>>>(a);
+        if (obs_only) k_bonds<VEC, kRS, false><<<grid, kBondsWarps * 32, 0, st>>>(a);
+        else k_bonds<VEC, kRS, true><<<grid, kBondsWarps * 32, 0, st>>>(a);
+    }
+    static void label(const SweepArgs &a, cudaStream_t st)
+    {
+        k_label<VEC, R, NW, LabelT><<<a.ntiles, NW * 32, 0, st>>>(a);
     }
     static void merge(const SweepArgs &a, cudaStream_t st)
     {
@@ -91,25 +100,23 @@ struct KS {
     {
         k_flip<VEC, R, NW, LabelT><<<grid, NW * 32, 0, st>>>(a);
     }
-    static int occupancy(int *bl_sweep, int *bl_obs, int *bl_label, int *fl)
+    static int occupancy(int *bonds_sweep, int *bonds_obs, int *fl)
     {
         cudaError_t e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bl_sweep, k_bonds_label<VEC, R, NW, LabelT, MODE_SWEEP>, NW * 32, 0);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_sweep, k_bonds<VEC, kRS, true>, kBondsWarps * 32, 0);
         if (e != cudaSuccess) return (int)e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bl_obs, k_bonds_label<VEC, R, NW, LabelT, MODE_OBS_ONLY>, NW * 32, 0);
-        if (e != cudaSuccess) return (int)e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bl_label, k_bonds_label<VEC, R, NW, LabelT, MODE_LABEL_ONLY>, NW * 32, 0);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_obs, k_bonds<VEC, kRS, false>, kBondsWarps * 32, 0);
         if (e != cudaSuccess) return (int)e;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(fl, k_flip<VEC, R, NW, LabelT>, NW * 32, 0);
         return (int)e;
     }
     static Kernels get()
     {
-        return Kernels{&bonds_label, &merge, &flip, &occupancy, 32 * VEC, R * NW, NW * 32};
+        return Kernels{&bonds, &label, &merge, &flip, &occupancy, 32 * VEC, R * NW, kRS};
     }
 };
 
-constexpr int kR = 8, kNW = 8;   // 8 warps x 8 rows: tiles of 128 x 64 (VEC 4) or 64 x 64 (VEC 2)
+constexpr int kR = 8, kNW = 8;   // label / flip tiles: 8 warps x 8 rows = 128 x 64 (VEC 4) or 64 x 64 (VEC 2)
 
 Kernels pick_kernels(uint32_t L, bool l64)
 {
@@ -194,7 +201,7 @@ struct xy_state {
     char *ws = nullptr;
     Layout lay{};
     Kernels ker{};
-    int grid_bl = 0, grid_fl = 0;
+    int grid_bonds = 0, grid_fl = 0;
     cudaStream_t stream = nullptr;
     bool have_sweep = false;        // bonds / labels of a sweep exist
     bool labels_flat = false;
@@ -203,6 +210,13 @@ struct xy_state {
     bool fix_phi = false;
     double phi_fixed = 0.0;
     void *stage = nullptr;          // lazily allocated device staging for the getters
+    uint64_t launches = 0;          // kernels launched so far
+    // per-kernel timing (xy_debug_kernel_timing)
+    bool timing = false;
+    std::vector<cudaEvent_t> ev;    // 4 events per timed sweep
+    size_t ev_used = 0;
+    double t_ms[4] = {0, 0, 0, 0};
+    uint64_t t_n[4] = {0, 0, 0, 0};
 
     float *theta() const { return reinterpret_cast<float *>(ws + lay.theta); }
     void *labels() const { return ws + lay.labels; }
@@ -210,6 +224,7 @@ struct xy_state {
     double *partials() const { return reinterpret_cast<double *>(ws + lay.partials); }
     xy_obs *ring() const { return reinterpret_cast<xy_obs *>(ws + lay.ring); }
     DevCtl *ctl() const { return reinterpret_cast<DevCtl *>(ws + lay.ctl); }
+    double2 *tab() const { return reinterpret_cast<double2 *>(ws + lay.tab); }
     bool l64() const { return (flags & XY_FLAG_LABELS64) != 0; }
 };
 
@@ -245,6 +260,7 @@ SweepArgs base_args(const xy_state *s)
     a.seed_lo = (uint32_t)(s->seed & 0xffffffffu);
     a.seed_hi = (uint32_t)(s->seed >> 32);
     a.t = (uint32_t)s->T;
+    a.sincos_tab = s->tab();
     return a;
 }
 
@@ -280,9 +296,40 @@ int ensure_obs(xy_state *s, int feed_pcc)
     SweepArgs a = base_args(s);
     a.obs_fill = 1;
     a.feed_pcc = feed_pcc;
-    s->ker.bonds_label(a, MODE_OBS_ONLY, s->grid_bl, s->stream);
+    s->ker.bonds(a, true, s->grid_bonds, s->stream);
     CUDA_TRY(cudaGetLastError());
+    s->launches += 1;
     s->obs_valid_T = s->T;
+    return XY_OK;
+}
+
+constexpr size_t kTimedSweepsPerFlush = 1024;
+constexpr int kTimedKernels = 4;      // k_bonds, k_label, k_merge, k_flip
+
+int timing_flush(xy_state *s)
+{
+    if (s->ev_used == 0) return XY_OK;
+    CUDA_TRY(cudaEventSynchronize(s->ev[s->ev_used - 1]));
+    for (size_t k = 0; k + kTimedKernels + 1 <= s->ev_used; k += kTimedKernels + 1) {
+        for (int j = 0; j < kTimedKernels; ++j) {
+            float ms = 0;
+            CUDA_TRY(cudaEventElapsedTime(&ms, s->ev[k + j], s->ev[k + j + 1]));
+            s->t_ms[j] += ms;
+            s->t_n[j] += 1;
+        }
+    }
+    s->ev_used = 0;
+    return XY_OK;
+}
+
+int timing_mark(xy_state *s)
+{
+    if (s->ev_used == s->ev.size()) {
+        cudaEvent_t e;
+        CUDA_TRY(cudaEventCreate(&e));
+        s->ev.push_back(e);
+    }
+    CUDA_TRY(cudaEventRecord(s->ev[s->ev_used++], s->stream));
     return XY_OK;
 }
 
@@ -296,10 +343,21 @@ int enqueue_sweep(xy_state *s, double beta, int beta_from_ctl, int feed_pcc)
     a.beta_from_ctl = beta_from_ctl;
     a.feed_pcc = feed_pcc;
     a.obs_fill = (s->obs_valid_T == s->T) ? 0 : 1;
-    s->ker.bonds_label(a, MODE_SWEEP, s->grid_bl, s->stream);
+    if (s->timing) {
+        if (s->ev_used >= (kTimedKernels + 1) * kTimedSweepsPerFlush)
+            if (int rc = timing_flush(s)) return rc;
+        if (int rc = timing_mark(s)) return rc;
+    }
+    s->ker.bonds(a, false, s->grid_bonds, s->stream);
+    if (s->timing) if (int rc = timing_mark(s)) return rc;
+    s->ker.label(a, s->stream);
+    if (s->timing) if (int rc = timing_mark(s)) return rc;
     s->ker.merge(a, s->stream);
+    if (s->timing) if (int rc = timing_mark(s)) return rc;
     s->ker.flip(a, s->grid_fl, s->stream);
+    if (s->timing) if (int rc = timing_mark(s)) return rc;
     CUDA_TRY(cudaGetLastError());
+    s->launches += 4;
     if (a.obs_fill) s->obs_valid_T = s->T;
     s->T += 1;
     if (s->T - s->oldest_T >= kRingCap) s->oldest_T = s->T - kRingCap + 1;
@@ -357,26 +415,45 @@ int xy_create_ex(xy_state **out, uint32_t L, uint64_t seed, int init, uint32_t f
         s->ws = static_cast<char *>(p);
         s->owns_ws = true;
     }
-    int bl = 0, bo = 0, blab = 0, fl = 0, sms = 0;
-    cudaError_t e = (cudaError_t)s->ker.occupancy(&bl, &bo, &blab, &fl);
+    int bs = 0, bo = 0, fl = 0, sms = 0;
+    cudaError_t e = (cudaError_t)s->ker.occupancy(&bs, &bo, &fl);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device);
-    if (e != cudaSuccess || bl < 1 || bo < 1 || blab < 1 || fl < 1) {
+    if (e != cudaSuccess || bs < 1 || bo < 1 || fl < 1) {
         if (s->owns_ws) cudaFree(s->ws);
         delete s;
         return fail(XY_ERR_CUDA, "kernel occupancy query failed: %s (was the library built for this GPU's sm_100a?)",
                     cudaGetErrorString(e));
     }
     const uint32_t ntiles = (L / s->ker.tw) * (L / s->ker.th);
-    // the three modes of k_bonds_label share ONE grid so that their fixed-order sums agree bitwise
-    int per_sm = bl < bo ? bl : bo;
-    if (blab < per_sm) per_sm = blab;
-    long g = (long)sms * per_sm;
-    if (g > (long)ntiles) g = ntiles;
+    const uint32_t nstrips = (L / s->ker.tw) * (L / s->ker.rs);
+    // both variants of k_bonds share ONE grid so that their fixed-order sums agree bitwise
+    long g = (long)sms * (bs < bo ? bs : bo);
+    const long need = (nstrips + kBondsWarps - 1) / kBondsWarps;
+    if (g > need) g = need;
     if (g > (long)kMaxGrid) g = kMaxGrid;
-    s->grid_bl = (int)g;
+    s->grid_bonds = (int)g;
     g = (long)sms * fl;
     if (g > (long)ntiles) g = ntiles;
     s->grid_fl = (int)g;
+
+    // sincos table: (cos, sin)(2 pi k / 256), k = 0..256, correctly rounded by the host libm
+    {
+        double2 h[kTabN + 1];
+        for (int k = 0; k <= kTabN; ++k) {
+            const long double ang = 6.283185307179586476925286766559L * (long double)k / (long double)kTabN;
+            h[k].x = (double)cosl(ang);
+            h[k].y = (double)sinl(ang);
+        }
+        h[0].x = 1.0; h[0].y = 0.0; h[kTabN].x = 1.0; h[kTabN].y = 0.0;
+        h[kTabN / 2].x = -1.0; h[kTabN / 2].y = 0.0;
+        h[kTabN / 4].x = 0.0; h[kTabN / 4].y = 1.0; h[3 * kTabN / 4].x = 0.0; h[3 * kTabN / 4].y = -1.0;
+        e = cudaMemcpy(s->tab(), h, sizeof h, cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) {
+            if (s->owns_ws) cudaFree(s->ws);
+            delete s;
+            return fail(XY_ERR_CUDA, "table upload failed: %s", cudaGetErrorString(e));
+        }
+    }
 
     if (init == XY_INIT_COLD) {
         e = cudaMemsetAsync(s->theta(), 0, s->N * 4, nullptr);
@@ -408,9 +485,36 @@ int xy_destroy(xy_state *s)
     if (!s) return XY_OK;
     DeviceGuard g(s->device);
     cudaStreamSynchronize(s->stream);
+    for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
     if (s->stage) cudaFree(s->stage);
     if (s->owns_ws) cudaFree(s->ws);
     delete s;
+    return XY_OK;
+}
+
+int xy_debug_kernel_timing(xy_state *s, int on)
+{
+    if (!s) return fail(XY_ERR_ARG, "state is NULL");
+    DeviceGuard g(s->device);
+    if (int rc = timing_flush(s)) return rc;
+    s->timing = on != 0;
+    if (on) for (int j = 0; j < kTimedKernels; ++j) { s->t_ms[j] = 0; s->t_n[j] = 0; }
+    return XY_OK;
+}
+
+int xy_get_kernel_times(xy_state *s, double ms[4], uint64_t launches[4])
+{
+    if (!s || !ms || !launches) return fail(XY_ERR_ARG, "NULL argument");
+    DeviceGuard g(s->device);
+    if (int rc = timing_flush(s)) return rc;
+    for (int j = 0; j < kTimedKernels; ++j) { ms[j] = s->t_ms[j]; launches[j] = s->t_n[j]; s->t_ms[j] = 0; s->t_n[j] = 0; }
+    return XY_OK;
+}
+
+int xy_get_launch_count(xy_state *s, uint64_t *count)
+{
+    if (!s || !count) return fail(XY_ERR_ARG, "NULL argument");
+    *count = s->launches;
     return XY_OK;
 }
 
@@ -653,8 +757,9 @@ int xy_label_bonds(xy_state *s, const uint8_t *host_bonds, size_t n)
         CUDA_TRY(cudaStreamSynchronize(s->stream));
     }
     SweepArgs a = base_args(s);
-    s->ker.bonds_label(a, MODE_LABEL_ONLY, s->grid_bl, s->stream);
+    s->ker.label(a, s->stream);
     s->ker.merge(a, s->stream);
+    s->launches += 2;
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaStreamSynchronize(s->stream));
     s->have_sweep = true;

@@ -1,15 +1,16 @@
 // xy_kernels.cuh -- the kernels of one Swendsen-Wang sweep of the 2D XY model on sm_100a.
 //
-//   k_bonds_label  (S2+S3, and S7 of the previous sweep): persistent CTAs walk TW x TH tiles.
-//                  Per tile: theta tile + halo -> fp64 (cos, sin, sigma) per site in registers ->
-//                  observables of the incoming configuration, Philox bond draws, filtered bond
-//                  decisions, run starts by ballot/clz over the x-bond bits, union-find over the
-//                  runs in shared memory -> provisional label (global index of the tile-local
-//                  root) + packed bond bits.  theta is read once (+ halo), labels written once.
+//   k_bonds   (S2, and S7 of the incoming configuration): warps stream strips of the lattice row
+//             by row: theta -> fp64 (cos, sin, sigma) per site in registers (table + short Taylor
+//             rotation) -> observables, Philox bond draws, filtered bond decisions -> packed bond
+//             bits (0.25 B/site).  theta is read once (+ halo); no block barrier in the loop.
+//   k_label   (S3): one CTA per TW x TH tile, integer only: run starts by ballot/clz over the
+//             x-bond bits, union-find over the runs in shared memory -> provisional label (global
+//             index of the tile-local root), written once.
 //   k_merge        (S4): one thread per tile-edge bond; atomicMin union-find on the label array.
 //   k_flip         (S5+S6): chase each site's label to the cluster's root (minimum site index),
 //                  draw the root's coin with Philox, reflect, write theta back.
-//   finalize       (S8): the last CTA of k_bonds_label reduces the per-CTA partial sums in a fixed
+//   finalize       (S8): the last CTA of k_bonds reduces the per-CTA partial sums in a fixed
 //                  order, writes the per-sweep record and advances the PCC controller.
 //
 // Layouts: theta fp32 row-major i = y*L + x.  labels LabelT (u32 or u64) same indexing.
@@ -40,7 +41,7 @@ struct DevCtl {
     unsigned long long trace_cap;
     // misc
     unsigned long long fallback_count;
-    unsigned int ticket;          // last-block-done counter of k_bonds_label
+    unsigned int ticket;          // last-block-done counter of k_bonds
     unsigned int pad;
 };
 
@@ -61,9 +62,9 @@ struct SweepArgs {
     int          obs_fill;        // 1: finalize writes the observables of the incoming state into ring[T]
     double       beta;
     double       phi, cphi, sphi, A;
+    const double2 *sincos_tab;    // [257] (cos, sin)(2 pi k / 256), host-computed
 };
 
-enum { MODE_SWEEP = 0, MODE_OBS_ONLY = 1, MODE_LABEL_ONLY = 2 };
 
 template <int VEC> struct FVec;
 template <> struct FVec<4> { using type = float4; };
@@ -129,22 +130,44 @@ __device__ inline void pcc_feed(DevCtl *c, double N, double Cx, double Sx, doubl
 }
 
 // ---------------------------------------------------------------------------------------------
-// k_bonds_label
+// k_bonds (S2, and S7 of the incoming configuration): streaming, no block barrier in the loop.
+// A warp walks strips of TW = 32*VEC columns x RS rows, top to bottom, one row per iteration,
+// carrying the previous row's (cos, sin, sigma) in registers; lane l owns VEC consecutive sites.
+// Right neighbour of a lane's last site: shuffle from lane+1; for lane 31 the strip's halo column,
+// computed once per strip by lanes 0..RS-1 into a per-warp shared slot.  Row RS of the strip (the
+// first row of the strip below) is recomputed as the y-halo (1/RS overhead).
 // ---------------------------------------------------------------------------------------------
-template <int VEC, int R, int NW, typename LabelT, int MODE>
-__global__ void __launch_bounds__(NW * 32, 2)
-k_bonds_label(const SweepArgs a)
-{
-    constexpr int TW = 32 * VEC;           // tile width  (sites)
-    constexpr int TH = R * NW;             // tile height (sites)
-    constexpr uint32_t VMASK = (1u << VEC) - 1u;
-    constexpr bool kObs = (MODE != MODE_LABEL_ONLY);
-    constexpr bool kLabel = (MODE != MODE_OBS_ONLY);
-    constexpr bool kFromTheta = (MODE != MODE_LABEL_ONLY);
+constexpr int kTabN = 256;                 // sincos table: entries k = 0..256 at angle 2 pi k / 256
 
-    __shared__ uint32_t parent[kLabel ? TW * TH : 1];
-    __shared__ double h_c[TH], h_s[TH], h_g[TH];      // halo column (right neighbour of the last tile column)
-    __shared__ float h_t[TH];
+// sin, cos of an fp32 angle in [0, 2pi(1+1e-7)]: table lookup + degree-5/4 Taylor rotation in
+// fp64, |error| < 1e-15 (|x| <= pi/256: x^7/5040 = 8e-18, x^6/720 = 5e-15).
+__device__ __forceinline__ void sincos_tab(float theta, const double2 *tab, double &s, double &c)
+{
+    const double t = (double)theta;
+    const double kd = __fma_rn(t, 40.743665431525208, 6755399441055744.0);      // 256/(2 pi), round to integer
+    const int k = __double2loint(kd);
+    const double kf = kd - 6755399441055744.0;
+    double x = __fma_rn(-kf, 0.02454369260617026, t);                          // fl64(2 pi)/256, exact scaling
+    x = __fma_rn(-kf, 9.5675529620887e-19, x);                                  // (2 pi - fl64(2 pi))/256
+    const double2 cs = tab[k];
+    const double x2 = x * x;
+    const double sx = __fma_rn(x * x2, __fma_rn(x2, 8.3333333333333333e-3, -1.6666666666666667e-1), x);
+    const double dc = x2 * __fma_rn(x2, 4.1666666666666667e-2, -0.5);           // cos x - 1
+    c = __fma_rn(-cs.y, sx, __fma_rn(cs.x, dc, cs.x));
+    s = __fma_rn(cs.x, sx, __fma_rn(cs.y, dc, cs.y));
+}
+
+template <int VEC, int RS, bool kBonds>
+__global__ void __launch_bounds__(128, 4)
+k_bonds(const SweepArgs a)
+{
+    constexpr int NW = 4;
+    constexpr int TW = 32 * VEC;
+    static_assert(RS <= 32, "halo column is computed by one lane per row");
+
+    __shared__ double2 tab[kTabN + 1];
+    __shared__ double h_c[NW][RS], h_s[NW][RS], h_g[NW][RS];
+    __shared__ float h_t[NW][RS];
     __shared__ double red[NW][6];
     __shared__ unsigned long long redc[NW][2];
     __shared__ bool is_last;
@@ -152,7 +175,8 @@ k_bonds_label(const SweepArgs a)
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
     const uint32_t L = a.L;
-    LabelT *labels = reinterpret_cast<LabelT *>(a.labels);
+    for (int k = threadIdx.x; k <= kTabN; k += blockDim.x) tab[k] = a.sincos_tab[k];
+    __syncthreads();
 
     double beta = a.beta;
     if (a.beta_from_ctl) beta = *reinterpret_cast<const volatile double *>(&a.ctl->beta);
@@ -161,228 +185,113 @@ k_bonds_label(const SweepArgs a)
     bcx.beta = beta;
     bcx.m2b = (float)(-2.0 * beta * 1.4426950408889634);
     bcx.fallback_counter = &a.ctl->fallback_count;
+    const double cphi = a.cphi, sphi = a.sphi;
 
     double aMx = 0, aMy = 0, aCx = 0, aSx = 0, aCy = 0, aSy = 0;
     uint32_t nbx = 0, nby = 0;
 
-    for (uint32_t tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
-        const uint32_t ty = tile / a.tiles_x, tx = tile - ty * a.tiles_x;
-        const uint32_t x0 = tx * TW, y0 = ty * TH;
-        const uint32_t xl = x0 + lane * VEC;                 // first column of this lane
-
-        // ---- loads: R+1 rows of VEC sites for this lane (row R is the halo row of the strip) ----
-        float tv[R + 1][VEC];
-        if constexpr (kFromTheta) {
-#pragma unroll
-            for (int r = 0; r <= R; ++r) {
-                uint32_t y = y0 + warp * R + r;
-                if (y >= L) y -= L;
-                load_vec<VEC, true>(a.theta + (size_t)y * L + xl, tv[r]);
-            }
-            // halo column: right neighbour of the tile's last column, rows 0..TH-1
-            if (threadIdx.x < TH) {
-                uint32_t xh = x0 + TW;
-                if (xh >= L) xh = 0;
-                const float th = __ldg(a.theta + (size_t)(y0 + threadIdx.x) * L + xh);
-                double s, c;
-                sincos_poly(th, s, c);
-                h_t[threadIdx.x] = th;
-                h_c[threadIdx.x] = c;
-                h_s[threadIdx.x] = s;
-                h_g[threadIdx.x] = __fma_rn(c, a.cphi, s * a.sphi);
-            }
+    const uint32_t strips_x = L / TW;
+    const uint32_t nstrips = strips_x * (L / RS);
+    for (uint32_t strip = blockIdx.x * NW + warp; strip < nstrips; strip += gridDim.x * NW) {
+        const uint32_t sy = strip / strips_x, sx = strip - sy * strips_x;
+        const uint32_t y0 = sy * RS;
+        const uint32_t xl = sx * TW + lane * VEC;
+        // halo column (right neighbour of the strip's last column), one lane per row
+        __syncwarp();
+        if (lane < RS) {
+            uint32_t xh = sx * TW + TW;
+            if (xh >= L) xh = 0;
+            const float th = __ldg(a.theta + (size_t)(y0 + lane) * L + xh);
+            double s, c;
+            sincos_tab(th, tab, s, c);
+            h_t[warp][lane] = th;
+            h_c[warp][lane] = c;
+            h_s[warp][lane] = s;
+            h_g[warp][lane] = __fma_rn(c, cphi, s * sphi);
         }
-        __syncthreads();   // (A) halo visible; previous tile's parent[] no longer in use
+        __syncwarp();
 
-        double pc[VEC] = {}, ps[VEC] = {}, pg[VEC] = {};   // previous row: cos, sin, sigma
-        uint32_t pwy[VEC] = {};                   // previous row: Philox words of the y bonds
-        uint32_t pstart[VEC] = {};                // previous row: run starts (local index)
-        uint32_t pxl = 0;                         // previous row: tile-local x bits
-        uint32_t pxn = 0;                         // previous row: all x bits (incl. the tile-crossing one)
-        uint32_t ylast = 0;                       // y bits of the strip's last row (cross-strip / tile edge)
+        float pt[VEC], nt[VEC];
+        double pc[VEC], ps[VEC], pg[VEC];
+        load_vec<VEC, true>(a.theta + (size_t)y0 * L + xl, pt);
+        {
+            uint32_t y1 = y0 + 1;
+            if (y1 >= L) y1 -= L;
+            load_vec<VEC, true>(a.theta + (size_t)y1 * L + xl, nt);
+        }
 #pragma unroll
-        for (int r = 0; r <= R; ++r) {
-            const int ly = warp * R + r;          // local row (== TH for the last warp's halo row)
-            uint32_t gy = y0 + ly;
-            if (gy >= L) gy -= L;
-            double c[VEC] = {}, s[VEC] = {}, g[VEC] = {};
-            uint32_t wx[VEC] = {}, wy[VEC] = {};
-            uint32_t xn = 0, yn = 0;              // x bits of row r, y bits of row r-1
-            if constexpr (kFromTheta) {
+        for (int v = 0; v < VEC; ++v) {
+            sincos_tab(pt[v], tab, ps[v], pc[v]);
+            pg[v] = __fma_rn(pc[v], cphi, ps[v] * sphi);
+        }
+#pragma unroll 1
+        for (int r = 1; r <= RS; ++r) {
+            // this iteration finishes row r-1 (held in p*): its x bonds, and its y bonds with row r
+            float ct[VEC];
 #pragma unroll
-                for (int v = 0; v < VEC; ++v) {
-                    sincos_poly(tv[r][v], s[v], c[v]);
-                    g[v] = __fma_rn(c[v], a.cphi, s[v] * a.sphi);
-                }
-                if (r < R) {
-                    // right neighbour of the lane's last site
-                    double cn = __shfl_down_sync(0xffffffffu, c[0], 1);
-                    double sn = __shfl_down_sync(0xffffffffu, s[0], 1);
-                    double gn = __shfl_down_sync(0xffffffffu, g[0], 1);
-                    float tn = __shfl_down_sync(0xffffffffu, tv[r][0], 1);
-                    if (lane == 31) { cn = h_c[ly]; sn = h_s[ly]; gn = h_g[ly]; tn = h_t[ly]; }
-                    if constexpr (kLabel) {
-#pragma unroll
-                        for (int v = 0; v < VEC; v += 2) {
-                            const uint64_t site = (uint64_t)gy * L + xl + v;
-                            const U4 w = rng(a.seed_lo, a.seed_hi, site >> 1, a.t, TAG_BOND);
-                            wx[v] = w.x; wy[v] = w.y; wx[v + 1] = w.z; wy[v + 1] = w.w;
-                        }
-                    }
-#pragma unroll
-                    for (int v = 0; v < VEC; ++v) {
-                        const double c2 = (v + 1 < VEC) ? c[(v + 1) % VEC] : cn;
-                        const double s2 = (v + 1 < VEC) ? s[(v + 1) % VEC] : sn;
-                        const double g2 = (v + 1 < VEC) ? g[(v + 1) % VEC] : gn;
-                        const float t2 = (v + 1 < VEC) ? tv[r][(v + 1) % VEC] : tn;
-                        if constexpr (kObs) {
-                            aMx += c[v];
-                            aMy += s[v];
-                            aCx = __fma_rn(c[v], c2, aCx);
-                            aCx = __fma_rn(s[v], s2, aCx);
-                            aSx = __fma_rn(s[v], c2, aSx);
-                            aSx = __fma_rn(-c[v], s2, aSx);
-                        }
-                        if constexpr (kLabel) {
-                            if (bond_decide(g[v] * g2, wx[v], tv[r][v], t2, bcx)) xn |= 1u << v;
-                        }
-                    }
-                }
-                if (r >= 1) {
-#pragma unroll
-                    for (int v = 0; v < VEC; ++v) {
-                        if constexpr (kObs) {
-                            aCy = __fma_rn(pc[v], c[v], aCy);
-                            aCy = __fma_rn(ps[v], s[v], aCy);
-                            aSy = __fma_rn(ps[v], c[v], aSy);
-                            aSy = __fma_rn(-pc[v], s[v], aSy);
-                        }
-                        if constexpr (kLabel) {
-                            if (bond_decide(pg[v] * g[v], pwy[v], tv[r - 1][v], tv[r][v], bcx)) yn |= 1u << v;
-                        }
-                    }
-                }
-            } else {
-                // LABEL_ONLY: bond bits injected through the packed bonds array
-                if (r < R) {
-                    uint32_t byte;
-                    if constexpr (VEC == 4) byte = a.bonds[((size_t)gy * L + xl) >> 2];
-                    else byte = a.bonds[((size_t)gy * L + xl) >> 2] >> ((lane & 1) * 2) & 0x33u;
-                    if constexpr (VEC == 4) { xn = byte & 15u; wy[0] = byte >> 4; }
-                    else { xn = byte & 3u; wy[0] = (byte >> 4) & 3u; }
-                }
-                if (r >= 1) yn = pwy[0];
+            for (int v = 0; v < VEC; ++v) ct[v] = nt[v];
+            if (r < RS) {                                   // prefetch row r+1
+                uint32_t y2 = y0 + r + 1;
+                if (y2 >= L) y2 -= L;
+                load_vec<VEC, true>(a.theta + (size_t)y2 * L + xl, nt);
             }
-
-            if constexpr (kLabel) {
-                // ---- record row r-1's bits (now complete) ----
-                if (r >= 1) {
-                    nbx += __popc(pxn);
-                    nby += __popc(yn);
-                    if constexpr (kFromTheta) {
-                        uint32_t py = gy == 0 ? L - 1 : gy - 1;
-                        if constexpr (VEC == 4) {
-                            a.bonds[((size_t)py * L + xl) >> 2] = (uint8_t)(pxn | (yn << 4));
-                        } else {
-                            // two lanes share a byte: even lane holds sites 4k,4k+1; odd lane 4k+2,4k+3
-                            const uint32_t mine = pxn | (yn << 4);
-                            const uint32_t other = __shfl_xor_sync(0xffffffffu, mine, 1);
-                            if ((lane & 1) == 0)
-                                a.bonds[((size_t)py * L + xl) >> 2] = (uint8_t)(mine | (other << 2));
-                        }
-                    }
-                }
-                uint32_t start[VEC] = {};
-                uint32_t xloc = 0;
-                if (r < R) {
-                    // ---- run starts of row r from the tile-local x bits ----
-                    xloc = xn;
-                    if (lane == 31) xloc &= ~(1u << (VEC - 1));          // that bond leaves the tile
-                    const uint32_t through = __ballot_sync(0xffffffffu, xloc == VMASK);
-                    const uint32_t lower = (1u << lane) - 1u;
-                    const uint32_t stop = ~through & lower;              // lanes below me that break the run
-                    const int lp = stop ? 31 - __clz(stop) : 0;
-                    const uint32_t nib = __shfl_sync(0xffffffffu, xloc, lp);
-                    uint32_t s0 = 0;
-                    if (stop) {
-                        const uint32_t zeros = ~nib & VMASK;             // non-empty: lane lp is not "through"
-                        s0 = lp * VEC + (31 - __clz(zeros)) + 1;
-                    }
-                    start[0] = ly * TW + s0;
-#pragma unroll
-                    for (int v = 1; v < VEC; ++v)
-                        start[v] = ((xloc >> (v - 1)) & 1u) ? start[v - 1] : (uint32_t)(ly * TW + lane * VEC + v);
-                    if constexpr (VEC == 4)
-                        *reinterpret_cast<uint4 *>(&parent[ly * TW + lane * 4]) = make_uint4(start[0], start[1], start[2], start[3]);
-                    else
-                        *reinterpret_cast<uint2 *>(&parent[ly * TW + lane * 2]) = make_uint2(start[0], start[1]);
-                }
-                // ---- vertical unions row r-1 -> r inside the strip ----
-                if (r >= 1 && r < R) {
-                    __syncwarp();
-                    // skip the bond if the left neighbour does the same union: it is joined to me
-                    // in both rows and has its own y bond
-                    const uint32_t packed = pxl | (xloc << 4) | (yn << 8);
-                    const uint32_t left = __shfl_up_sync(0xffffffffu, packed, 1);
-                    const bool lconn = lane > 0 && ((left >> (VEC - 1)) & 1u) && ((left >> (4 + VEC - 1)) & 1u) &&
-                                       ((left >> (8 + VEC - 1)) & 1u);
-#pragma unroll
-                    for (int v = 0; v < VEC; ++v) {
-                        if ((yn >> v) & 1u) {
-                            const bool dup = v == 0 ? lconn
-                                                    : (((pxl >> (v - 1)) & 1u) && ((xloc >> (v - 1)) & 1u) && ((yn >> (v - 1)) & 1u));
-                            if (!dup) sunion(parent, pstart[v], start[v]);
-                        }
-                    }
-                    __syncwarp();
-                }
-                if (r == R) ylast = yn;
-#pragma unroll
-                for (int v = 0; v < VEC; ++v) pstart[v] = start[v];
-                pxl = xloc;
-                pxn = xn;
-            }
+            double c[VEC], s[VEC], g[VEC];
 #pragma unroll
             for (int v = 0; v < VEC; ++v) {
-                pc[v] = c[v]; ps[v] = s[v]; pg[v] = g[v];
-                pwy[v] = wy[v];
+                sincos_tab(ct[v], tab, s[v], c[v]);
+                g[v] = __fma_rn(c[v], cphi, s[v] * sphi);
             }
-        }
-
-        if constexpr (kLabel) {
-            __syncthreads();   // (B) every strip's parents are in place
-            if (warp < NW - 1) {
-                const int ly = warp * R + R - 1;
+            const uint32_t gy = y0 + r - 1;                 // global row being finished
+            double cn = __shfl_down_sync(0xffffffffu, pc[0], 1);
+            double sn = __shfl_down_sync(0xffffffffu, ps[0], 1);
+            double gn = __shfl_down_sync(0xffffffffu, pg[0], 1);
+            float tn = __shfl_down_sync(0xffffffffu, pt[0], 1);
+            if (lane == 31) { cn = h_c[warp][r - 1]; sn = h_s[warp][r - 1]; gn = h_g[warp][r - 1]; tn = h_t[warp][r - 1]; }
+            uint32_t wx[VEC], wy[VEC];
+            if constexpr (kBonds) {
 #pragma unroll
-                for (int v = 0; v < VEC; ++v)
-                    if ((ylast >> v) & 1u)
-                        sunion(parent, (uint32_t)(ly * TW + lane * VEC + v), (uint32_t)((ly + 1) * TW + lane * VEC + v));
-            }
-            __syncthreads();   // (C) tile-local forest complete
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const int ly = warp * R + r;
-                LabelT out[VEC];
-                uint32_t prev_p = 0xffffffffu, prev_root = 0;
-#pragma unroll
-                for (int v = 0; v < VEC; ++v) {
-                    const uint32_t p = parent[ly * TW + lane * VEC + v];
-                    const uint32_t root = (p == prev_p) ? prev_root : sfind(parent, p);
-                    prev_p = p;
-                    prev_root = root;
-                    const uint32_t ry = root / TW, rx = root - ry * TW;
-                    out[v] = (LabelT)(y0 + ry) * L + (x0 + rx);
+                for (int v = 0; v < VEC; v += 2) {
+                    const uint64_t site = (uint64_t)gy * L + xl + v;
+                    const U4 w = rng(a.seed_lo, a.seed_hi, site >> 1, a.t, TAG_BOND);
+                    wx[v] = w.x; wy[v] = w.y; wx[v + 1] = w.z; wy[v + 1] = w.w;
                 }
-                LabelT *dst = labels + (size_t)(y0 + ly) * L + xl;
-                if constexpr (sizeof(LabelT) == 4) {
-                    if constexpr (VEC == 4) *reinterpret_cast<uint4 *>(dst) = make_uint4(out[0], out[1], out[2], out[3]);
-                    else *reinterpret_cast<uint2 *>(dst) = make_uint2(out[0], out[1]);
+            }
+            uint32_t xn = 0, yn = 0;
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) {
+                const double c2 = (v + 1 < VEC) ? pc[(v + 1) % VEC] : cn;
+                const double s2 = (v + 1 < VEC) ? ps[(v + 1) % VEC] : sn;
+                const double g2 = (v + 1 < VEC) ? pg[(v + 1) % VEC] : gn;
+                const float t2 = (v + 1 < VEC) ? pt[(v + 1) % VEC] : tn;
+                aMx += pc[v];
+                aMy += ps[v];
+                aCx = __fma_rn(pc[v], c2, aCx);
+                aCx = __fma_rn(ps[v], s2, aCx);
+                aSx = __fma_rn(ps[v], c2, aSx);
+                aSx = __fma_rn(-pc[v], s2, aSx);
+                aCy = __fma_rn(pc[v], c[v], aCy);
+                aCy = __fma_rn(ps[v], s[v], aCy);
+                aSy = __fma_rn(ps[v], c[v], aSy);
+                aSy = __fma_rn(-pc[v], s[v], aSy);
+                if constexpr (kBonds) {
+                    if (bond_decide(pg[v] * g2, wx[v], pt[v], t2, bcx)) xn |= 1u << v;
+                    if (bond_decide(pg[v] * g[v], wy[v], pt[v], ct[v], bcx)) yn |= 1u << v;
+                }
+            }
+            if constexpr (kBonds) {
+                nbx += __popc(xn);
+                nby += __popc(yn);
+                if constexpr (VEC == 4) {
+                    a.bonds[((size_t)gy * L + xl) >> 2] = (uint8_t)(xn | (yn << 4));
                 } else {
-#pragma unroll
-                    for (int v = 0; v < VEC; v += 2)
-                        *reinterpret_cast<ulonglong2 *>(dst + v) = make_ulonglong2(out[v], out[v + 1]);
+                    // two lanes share a byte: even lane holds sites 4k,4k+1; odd lane 4k+2,4k+3
+                    const uint32_t mine = xn | (yn << 4);
+                    const uint32_t other = __shfl_xor_sync(0xffffffffu, mine, 1);
+                    if ((lane & 1) == 0) a.bonds[((size_t)gy * L + xl) >> 2] = (uint8_t)(mine | (other << 2));
                 }
             }
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) { pc[v] = c[v]; ps[v] = s[v]; pg[v] = g[v]; pt[v] = ct[v]; }
         }
     }
 
@@ -414,7 +323,7 @@ k_bonds_label(const SweepArgs a)
     __syncthreads();
     if (!is_last) return;
 
-    // ---- finalize (S8): last CTA reduces the partials in a fixed order ----
+    // ---- finalize (S8): the last CTA reduces the partials in a fixed order ----
     __threadfence();
     {
         double acc[6] = {0, 0, 0, 0, 0, 0};
@@ -441,15 +350,13 @@ k_bonds_label(const SweepArgs a)
                 b0 += redc[w][0]; b1 += redc[w][1];
             }
             const double N = (double)L * (double)L;
-            if constexpr (kObs) {
-                if (a.obs_fill) {
-                    xy_obs *o = a.ring + (a.t % a.ring_cap);     // record of T = t (the incoming state)
-                    o->Mx = tot[0]; o->My = tot[1]; o->Cx = tot[2]; o->Sx = tot[3]; o->Cy = tot[4]; o->Sy = tot[5];
-                    o->E = -(tot[2] + tot[4]);
-                }
-                if (a.feed_pcc) pcc_feed(a.ctl, N, tot[2], tot[3], tot[4], tot[5]);
+            if (a.obs_fill) {
+                xy_obs *o = a.ring + (a.t % a.ring_cap);         // record of T = t (the incoming state)
+                o->Mx = tot[0]; o->My = tot[1]; o->Cx = tot[2]; o->Sx = tot[3]; o->Cy = tot[4]; o->Sy = tot[5];
+                o->E = -(tot[2] + tot[4]);
             }
-            if constexpr (MODE == MODE_SWEEP) {
+            if (a.feed_pcc) pcc_feed(a.ctl, N, tot[2], tot[3], tot[4], tot[5]);
+            if constexpr (kBonds) {
                 xy_obs *o = a.ring + ((a.t + 1u) % a.ring_cap);  // record of T = t+1, completed later
                 o->sweep = (uint64_t)a.t + 1u;
                 o->beta = beta;
@@ -459,6 +366,125 @@ k_bonds_label(const SweepArgs a)
             }
             a.ctl->ticket = 0;
             __threadfence();
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// k_label (S3): tile-local labeling from the packed bond bits; integer only.  One CTA per
+// TW x TH tile (TW = 32*VEC, TH = R*NW).  Phase 1: run starts of every row by ballot/clz over the
+// x bits -> parent[].  Phase 2: one union per (pair of vertically adjacent runs joined by a y
+// bond), atomicMin in shared memory.  Phase 3: provisional label = global index of the
+// tile-local root.  Bonds that leave the tile are left to k_merge.
+// ---------------------------------------------------------------------------------------------
+template <int VEC, int R, int NW, typename LabelT>
+__global__ void __launch_bounds__(NW * 32)
+k_label(const SweepArgs a)
+{
+    constexpr int TW = 32 * VEC, TH = R * NW;
+    constexpr uint32_t VMASK = (1u << VEC) - 1u;
+    __shared__ uint32_t parent[TW * TH];
+    __shared__ uint8_t sb[TH][32];                // per row, per lane: tile-local x bits | y bits << 4
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t L = a.L;
+    LabelT *labels = reinterpret_cast<LabelT *>(a.labels);
+    const uint32_t tile = blockIdx.x;
+    const uint32_t ty = tile / a.tiles_x, tx = tile - ty * a.tiles_x;
+    const uint32_t x0 = tx * TW, y0 = ty * TH;
+    const uint32_t xl = x0 + lane * VEC;
+
+    // ---- phase 1: bits -> run starts ----
+    uint32_t bytes[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int ly = warp * R + r;
+        uint32_t b = a.bonds[((size_t)(y0 + ly) * L + xl) >> 2];
+        if constexpr (VEC == 2) b = (b >> ((lane & 1) * 2)) & 0x33u;
+        bytes[r] = b;
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int ly = warp * R + r;
+        uint32_t xloc = bytes[r] & VMASK;
+        uint32_t yn = (bytes[r] >> 4) & VMASK;
+        if (lane == 31) xloc &= ~(1u << (VEC - 1));              // that bond leaves the tile
+        if (ly == TH - 1) yn = 0;                                // those bonds leave the tile
+        const uint32_t through = __ballot_sync(0xffffffffu, xloc == VMASK);
+        const uint32_t lower = (1u << lane) - 1u;
+        const uint32_t stop = ~through & lower;                  // lanes below me that break the run
+        const int lp = stop ? 31 - __clz(stop) : 0;
+        const uint32_t nib = __shfl_sync(0xffffffffu, xloc, lp);
+        uint32_t s0 = 0;
+        if (stop) {
+            const uint32_t zeros = ~nib & VMASK;                 // non-empty: lane lp is not "through"
+            s0 = lp * VEC + (31 - __clz(zeros)) + 1;
+        }
+        uint32_t start[VEC];
+        start[0] = ly * TW + s0;
+#pragma unroll
+        for (int v = 1; v < VEC; ++v)
+            start[v] = ((xloc >> (v - 1)) & 1u) ? start[v - 1] : (uint32_t)(ly * TW + lane * VEC + v);
+        if constexpr (VEC == 4)
+            *reinterpret_cast<uint4 *>(&parent[ly * TW + lane * 4]) = make_uint4(start[0], start[1], start[2], start[3]);
+        else
+            *reinterpret_cast<uint2 *>(&parent[ly * TW + lane * 2]) = make_uint2(start[0], start[1]);
+        sb[ly][lane] = (uint8_t)(xloc | (yn << 4));
+        bytes[r] = xloc | (yn << 4);
+    }
+    __syncthreads();
+
+    // ---- phase 2: vertical unions ----
+    {
+        uint32_t need = 0;                                       // bit r*4+v: union (ly, v) with (ly+1, v)
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int ly = warp * R + r;
+            const uint32_t yn = bytes[r] >> 4;
+            if (yn == 0) continue;                               // also covers ly == TH-1
+            const uint32_t xu = bytes[r] & VMASK;                // my row's x bits
+            const uint32_t xd = sb[ly + 1][lane] & VMASK;        // the row below
+            // a bond is redundant if the left neighbour is joined to me in both rows and has its own y bond
+            uint32_t dup = (xu & xd & yn) << 1;
+            if (lane > 0) {
+                const uint32_t lu = sb[ly][lane - 1], ld = sb[ly + 1][lane - 1];
+                dup |= ((lu & ld & (lu >> 4)) >> (VEC - 1)) & 1u;
+            }
+            need |= (yn & ~dup & VMASK) << (r * 4);
+        }
+        while (need) {
+            const int bit = __ffs(need) - 1;
+            need &= need - 1;
+            const int ly = warp * R + (bit >> 2);
+            const uint32_t s = ly * TW + lane * VEC + (bit & 3);
+            sunion(parent, parent[s], parent[s + TW]);
+        }
+    }
+    __syncthreads();
+
+    // ---- phase 3: provisional labels ----
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int ly = warp * R + r;
+        LabelT out[VEC];
+        uint32_t prev_p = 0xffffffffu, prev_root = 0;
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) {
+            const uint32_t p = parent[ly * TW + lane * VEC + v];
+            const uint32_t root = (p == prev_p) ? prev_root : sfind(parent, p);
+            prev_p = p;
+            prev_root = root;
+            const uint32_t ry = root / TW, rx = root - ry * TW;
+            out[v] = (LabelT)(y0 + ry) * L + (x0 + rx);
+        }
+        LabelT *dst = labels + (size_t)(y0 + ly) * L + xl;
+        if constexpr (sizeof(LabelT) == 4) {
+            if constexpr (VEC == 4) *reinterpret_cast<uint4 *>(dst) = make_uint4(out[0], out[1], out[2], out[3]);
+            else *reinterpret_cast<uint2 *>(dst) = make_uint2(out[0], out[1]);
+        } else {
+#pragma unroll
+            for (int v = 0; v < VEC; v += 2)
+                *reinterpret_cast<ulonglong2 *>(dst + v) = make_ulonglong2(out[v], out[v + 1]);
         }
     }
 }
