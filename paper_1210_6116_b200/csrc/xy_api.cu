@@ -87,7 +87,13 @@ struct KS {
     }
     static void label(const SweepArgs &a, cudaStream_t st)
     {
-        k_label<VEC, R, NW, LabelT><<<a.ntiles, NW * 32, 0, st>>>(a);
+        static bool attr_set = false;
+        if (!attr_set) {
+            cudaFuncSetAttribute(k_label<VEC, R, NW, LabelT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)k_label_smem_bytes<VEC, R, NW>());
+            attr_set = true;
+        }
+        k_label<VEC, R, NW, LabelT><<<a.ntiles, NW * 32, k_label_smem_bytes<VEC, R, NW>(), st>>>(a);
     }
     static void merge(const SweepArgs &a, cudaStream_t st)
     {

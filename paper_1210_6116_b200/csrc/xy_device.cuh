@@ -144,16 +144,24 @@ __device__ __forceinline__ uint32_t sfind(const volatile uint32_t *p, uint32_t a
     return a;
 }
 
+// Both chains advance in lock step (two independent loads per round); a node that already is a
+// root re-reads itself.  Links go from the larger root to the smaller one.
 __device__ __forceinline__ void sunion(uint32_t *p, uint32_t a, uint32_t b)
 {
+    const volatile uint32_t *vp = p;
     for (;;) {
-        a = sfind(p, a);
-        b = sfind(p, b);
         if (a == b) return;
-        if (a < b) { const uint32_t t = a; a = b; b = t; }      // a > b: link a -> b
-        const uint32_t old = atomicMin(&p[a], b);
-        if (old == a) return;
-        a = old;                                                 // a was re-linked meanwhile: carry on with its parent
+        const uint32_t pa = vp[a], pb = vp[b];
+        if (pa == a && pb == b) {
+            const uint32_t hi = a > b ? a : b, lo = a > b ? b : a;
+            const uint32_t old = atomicMin(&p[hi], lo);
+            if (old == hi) return;
+            a = old;                                             // hi was re-linked meanwhile: carry on with its parent
+            b = lo;
+        } else {
+            a = pa;
+            b = pb;
+        }
     }
 }
 

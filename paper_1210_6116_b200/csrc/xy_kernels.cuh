@@ -372,19 +372,29 @@ k_bonds(const SweepArgs a)
 
 // ---------------------------------------------------------------------------------------------
 // k_label (S3): tile-local labeling from the packed bond bits; integer only.  One CTA per
-// TW x TH tile (TW = 32*VEC, TH = R*NW).  Phase 1: run starts of every row by ballot/clz over the
-// x bits -> parent[].  Phase 2: one union per (pair of vertically adjacent runs joined by a y
-// bond), atomicMin in shared memory.  Phase 3: provisional label = global index of the
-// tile-local root.  Bonds that leave the tile are left to k_merge.
+// TW x TH tile (TW = 32*VEC, TH = R*NW); warp w owns the strip of rows [w*R, (w+1)*R).
+//   scan   each warp walks its strip top to bottom, all lanes on the same row: run starts of the
+//          row by ballot/clz over the x bits -> parent[]; then every y bond that is not redundant
+//          ATTACHES the lower run's fresh root to the upper site's root, which the lane carries
+//          in registers: one atomicMin, no find.  Only when the run was already attached
+//          elsewhere (two upper components meet) a real union runs.  Row order keeps trees flat.
+//   stitch unions across the NW-1 strip boundaries (generic lock-step union).
+//   emit   provisional label = global index of the tile-local root (min index in the tile-local
+//          component).  Bonds that leave the tile are left to k_merge.
 // ---------------------------------------------------------------------------------------------
+template <int VEC, int R, int NW>
+constexpr size_t k_label_smem_bytes() { return (size_t)(32 * VEC) * (R * NW) * 4 + (size_t)NW * 64; }
+
 template <int VEC, int R, int NW, typename LabelT>
 __global__ void __launch_bounds__(NW * 32)
 k_label(const SweepArgs a)
 {
     constexpr int TW = 32 * VEC, TH = R * NW;
     constexpr uint32_t VMASK = (1u << VEC) - 1u;
-    __shared__ uint32_t parent[TW * TH];
-    __shared__ uint8_t sb[TH][32];                // per row, per lane: tile-local x bits | y bits << 4
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    uint32_t *parent = reinterpret_cast<uint32_t *>(smem_raw);                     // [TW*TH]
+    uint8_t (*xfirst)[32] = reinterpret_cast<uint8_t (*)[32]>(smem_raw + TW * TH * 4);          // x bits of each strip's first row
+    uint8_t (*xlast)[32] = reinterpret_cast<uint8_t (*)[32]>(smem_raw + TW * TH * 4 + NW * 32); // x | y << 4 bits of its last row
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t L = a.L;
@@ -394,32 +404,35 @@ k_label(const SweepArgs a)
     const uint32_t x0 = tx * TW, y0 = ty * TH;
     const uint32_t xl = x0 + lane * VEC;
 
-    // ---- phase 1: bits -> run starts ----
     uint32_t bytes[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-        const int ly = warp * R + r;
-        uint32_t b = a.bonds[((size_t)(y0 + ly) * L + xl) >> 2];
+        uint32_t b = a.bonds[((size_t)(y0 + warp * R + r) * L + xl) >> 2];
         if constexpr (VEC == 2) b = (b >> ((lane & 1) * 2)) & 0x33u;
         bytes[r] = b;
     }
+
+    // ---- scan ----
+    uint32_t rootU[VEC];            // root (as of the previous row) of the VEC sites above
+    uint32_t xprev = 0, yprev = 0;  // tile-local x bits and y bits of the previous row
 #pragma unroll
+    for (int v = 0; v < VEC; ++v) rootU[v] = 0;
+#pragma unroll 1
     for (int r = 0; r < R; ++r) {
         const int ly = warp * R + r;
-        uint32_t xloc = bytes[r] & VMASK;
-        uint32_t yn = (bytes[r] >> 4) & VMASK;
-        if (lane == 31) xloc &= ~(1u << (VEC - 1));              // that bond leaves the tile
-        if (ly == TH - 1) yn = 0;                                // those bonds leave the tile
+        uint32_t xloc = bytes[0] & VMASK;
+        const uint32_t yn = (bytes[0] >> 4) & VMASK;
+#pragma unroll
+        for (int k = 0; k + 1 < R; ++k) bytes[k] = bytes[k + 1];                 // rotate (keeps indices static)
+        if (lane == 31) xloc &= ~(1u << (VEC - 1));                              // that bond leaves the tile
+        if (r == 0) xfirst[warp][lane] = (uint8_t)xloc;
+        // run starts of this row
         const uint32_t through = __ballot_sync(0xffffffffu, xloc == VMASK);
-        const uint32_t lower = (1u << lane) - 1u;
-        const uint32_t stop = ~through & lower;                  // lanes below me that break the run
+        const uint32_t stop = ~through & ((1u << lane) - 1u);                    // lanes below me that break the run
         const int lp = stop ? 31 - __clz(stop) : 0;
         const uint32_t nib = __shfl_sync(0xffffffffu, xloc, lp);
         uint32_t s0 = 0;
-        if (stop) {
-            const uint32_t zeros = ~nib & VMASK;                 // non-empty: lane lp is not "through"
-            s0 = lp * VEC + (31 - __clz(zeros)) + 1;
-        }
+        if (stop) s0 = lp * VEC + (31 - __clz(~nib & VMASK)) + 1;
         uint32_t start[VEC];
         start[0] = ly * TW + s0;
 #pragma unroll
@@ -429,51 +442,92 @@ k_label(const SweepArgs a)
             *reinterpret_cast<uint4 *>(&parent[ly * TW + lane * 4]) = make_uint4(start[0], start[1], start[2], start[3]);
         else
             *reinterpret_cast<uint2 *>(&parent[ly * TW + lane * 2]) = make_uint2(start[0], start[1]);
-        sb[ly][lane] = (uint8_t)(xloc | (yn << 4));
-        bytes[r] = xloc | (yn << 4);
-    }
-    __syncthreads();
-
-    // ---- phase 2: vertical unions ----
-    {
-        uint32_t need = 0;                                       // bit r*4+v: union (ly, v) with (ly+1, v)
+        __syncwarp();
+        if (r > 0) {
+            // a y bond is redundant if the left neighbour is joined to me in both rows and has its own y bond
+            uint32_t dup = (xprev & xloc & yprev) << 1;
+            const uint32_t packed = xprev & xloc & yprev;
+            const uint32_t left = __shfl_up_sync(0xffffffffu, packed, 1);
+            if (lane > 0) dup |= (left >> (VEC - 1)) & 1u;
+            const uint32_t need = yprev & ~dup & VMASK;
+            // attach: the lower run's root takes the upper root unless it already has a smaller one
+            uint32_t fail = 0, other[VEC];
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const int ly = warp * R + r;
-            const uint32_t yn = bytes[r] >> 4;
-            if (yn == 0) continue;                               // also covers ly == TH-1
-            const uint32_t xu = bytes[r] & VMASK;                // my row's x bits
-            const uint32_t xd = sb[ly + 1][lane] & VMASK;        // the row below
-            // a bond is redundant if the left neighbour is joined to me in both rows and has its own y bond
-            uint32_t dup = (xu & xd & yn) << 1;
-            if (lane > 0) {
-                const uint32_t lu = sb[ly][lane - 1], ld = sb[ly + 1][lane - 1];
-                dup |= ((lu & ld & (lu >> 4)) >> (VEC - 1)) & 1u;
+            for (int v = 0; v < VEC; ++v) {
+                other[v] = 0;
+                if ((need >> v) & 1u) {
+                    const uint32_t old = atomicMin(&parent[start[v]], rootU[v]);
+                    if (old != start[v] && old != rootU[v]) { fail |= 1u << v; other[v] = old; }
+                }
             }
-            need |= (yn & ~dup & VMASK) << (r * 4);
+            // two upper components met in one lower run: real union (rare)
+            if (__any_sync(0xffffffffu, fail != 0)) {
+#pragma unroll
+                for (int v = 0; v < VEC; ++v)
+                    if ((fail >> v) & 1u) sunion(parent, other[v], rootU[v]);
+            }
+            __syncwarp();
         }
-        while (need) {
-            const int bit = __ffs(need) - 1;
-            need &= need - 1;
-            const int ly = warp * R + (bit >> 2);
-            const uint32_t s = ly * TW + lane * VEC + (bit & 3);
-            sunion(parent, parent[s], parent[s + TW]);
+        // roots of this row's sites for the next row (one extra hop against staleness)
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) {
+            const uint32_t p1 = (v > 0 && start[v] == start[v - 1]) ? rootU[v - 1] : parent[parent[start[v]]];
+            rootU[v] = p1;
+        }
+        xprev = xloc;
+        yprev = yn;
+    }
+
+    // ---- stitch: strip boundaries IN ORDER, by one warp.  When boundary w is processed the strips
+    //      0..w are already one forest whose roots are final for those strips, so every root of
+    //      strip w+1 links straight to a final root: chains stay site -> run start -> strip root -> root.
+    xlast[warp][lane] = (uint8_t)(xprev | (yprev << 4));
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll 1
+        for (int w = 0; w + 1 < NW; ++w) {
+            const uint32_t bu = xlast[w][lane], xu = bu & VMASK, yu = bu >> 4;
+            const uint32_t xd = xfirst[w + 1][lane];
+            const uint32_t packed = xu & xd & yu;
+            uint32_t dup = packed << 1;
+            const uint32_t left = __shfl_up_sync(0xffffffffu, packed, 1);
+            if (lane > 0) dup |= (left >> (VEC - 1)) & 1u;
+            const uint32_t need = yu & ~dup & VMASK;
+            const uint32_t above = (w * R + R - 1) * TW + lane * VEC;
+#pragma unroll
+            for (int v = 0; v < VEC; ++v)
+                if ((need >> v) & 1u) sunion(parent, parent[above + v], parent[above + TW + v]);
+            __syncwarp();
         }
     }
     __syncthreads();
 
-    // ---- phase 3: provisional labels ----
+    // ---- emit: provisional labels (three hops unrolled for all VEC sites, then the rare rest) ----
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int ly = warp * R + r;
+        uint32_t p0[VEC], p1[VEC];
+        if constexpr (VEC == 4) {
+            const uint4 q = *reinterpret_cast<const uint4 *>(&parent[ly * TW + lane * 4]);
+            p0[0] = q.x; p0[1] = q.y; p0[2] = q.z; p0[3] = q.w;
+        } else {
+            const uint2 q = *reinterpret_cast<const uint2 *>(&parent[ly * TW + lane * 2]);
+            p0[0] = q.x; p0[1] = q.y;
+        }
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) p1[v] = parent[p0[v]];
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) p0[v] = parent[p1[v]];
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) p1[v] = parent[p0[v]];
+        // now p0 = 2 hops above the site's run start, p1 = parent[p0]
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) { const uint32_t t = p0[v]; p0[v] = p1[v]; p1[v] = t; }
         LabelT out[VEC];
-        uint32_t prev_p = 0xffffffffu, prev_root = 0;
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
-            const uint32_t p = parent[ly * TW + lane * VEC + v];
-            const uint32_t root = (p == prev_p) ? prev_root : sfind(parent, p);
-            prev_p = p;
-            prev_root = root;
+            uint32_t root = p0[v];
+            if (root != p1[v]) root = sfind(parent, root);
             const uint32_t ry = root / TW, rx = root - ry * TW;
             out[v] = (LabelT)(y0 + ry) * L + (x0 + rx);
         }
