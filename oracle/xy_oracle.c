@@ -267,8 +267,10 @@ uint64_t xyo_label(const uint8_t *bonds, uint32_t L32, int64_t *label)
 }
 
 /* ------------------------------------------------------------------------- */
-/* O6. Flip.  Coin of a cluster f(rho) = top bit of rng(seed, rho, t, FLIP)[0] */
-/* with rho the cluster's canonical label.  A flipped site is reflected across */
+/* O6. Flip.  Coin of a cluster with canonical label rho: one Philox call    */
+/* serves 128 consecutive labels: f(rho) = bit (rho mod 128) of the 128-bit    */
+/* output of rng(seed, rho div 128, t, FLIP), i.e. bit (rho & 31) of word       */
+/* (rho >> 5) & 3.  A flipped site is reflected across                         */
 /* the line perpendicular to r:  theta -> 2 phi + pi - theta (mod 2 pi), i.e.  */
 /* s -> s - 2 (s.r) r.  Specified to the rounding: only fp64 add/sub and one   */
 /* fp64 -> fp32 conversion (round to nearest even).                            */
@@ -276,8 +278,8 @@ uint64_t xyo_label(const uint8_t *bonds, uint32_t L32, int64_t *label)
 int xyo_flip_coin(uint64_t seed, uint64_t rho, uint64_t t)
 {
     uint32_t w[4];
-    xyo_rng(seed, rho, t, XYO_TAG_FLIP, w);
-    return (int)(w[0] >> 31);
+    xyo_rng(seed, rho >> 7, t, XYO_TAG_FLIP, w);
+    return (int)((w[(rho >> 5) & 3u] >> (rho & 31u)) & 1u);
 }
 
 double xyo_reflect_const(double phi)

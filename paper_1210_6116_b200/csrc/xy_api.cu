@@ -45,7 +45,7 @@ constexpr size_t kStageBytes = 64u << 20;  // staging buffer of the debug getter
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-    size_t theta, labels, bonds, partials, ring, ctl, tab, total;
+    size_t theta, labels, bonds, rootmask, partials, ring, ctl, tab, total;
 };
 
 Layout make_layout(uint32_t L, uint32_t flags)
@@ -57,6 +57,7 @@ Layout make_layout(uint32_t L, uint32_t flags)
     o.theta = off;    off = align_up(off + N * 4, 256);
     o.labels = off;   off = align_up(off + N * lw, 256);
     o.bonds = off;    off = align_up(off + N / 4, 256);
+    o.rootmask = off; off = align_up(off + N / 8, 256);
     o.partials = off; off = align_up(off + (size_t)kMaxGrid * kPartialStride * 8, 256);
     o.ring = off;     off = align_up(off + (size_t)kRingCap * sizeof(xy_obs), 256);
     o.ctl = off;      off = align_up(off + sizeof(DevCtl), 256);
@@ -89,11 +90,11 @@ struct KS {
     {
         static bool attr_set = false;
         if (!attr_set) {
-            cudaFuncSetAttribute(k_label<VEC, R, NW, LabelT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)k_label_smem_bytes<VEC, R, NW>());
+            cudaFuncSetAttribute(k_label<VEC, R * NW, LabelT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)k_label_smem_bytes<VEC, R * NW>());
             attr_set = true;
         }
-        k_label<VEC, R, NW, LabelT><<<a.ntiles, NW * 32, k_label_smem_bytes<VEC, R, NW>(), st>>>(a);
+        k_label<VEC, R * NW, LabelT><<<a.ntiles, VEC * R * NW, k_label_smem_bytes<VEC, R * NW>(), st>>>(a);
     }
     static void merge(const SweepArgs &a, cudaStream_t st)
     {
@@ -104,7 +105,8 @@ struct KS {
     }
     static void flip(const SweepArgs &a, int grid, cudaStream_t st)
     {
-        k_flip<VEC, R, NW, LabelT><<<grid, NW * 32, 0, st>>>(a);
+        (void)grid;
+        k_flip<VEC, R * NW, LabelT><<<a.ntiles, VEC * R * NW, 0, st>>>(a);
     }
     static int occupancy(int *bonds_sweep, int *bonds_obs, int *fl)
     {
@@ -113,7 +115,7 @@ struct KS {
         if (e != cudaSuccess) return (int)e;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_obs, k_bonds<VEC, kRS, false>, kBondsWarps * 32, 0);
         if (e != cudaSuccess) return (int)e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(fl, k_flip<VEC, R, NW, LabelT>, NW * 32, 0);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(fl, k_flip<VEC, R * NW, LabelT>, VEC * R * NW, 0);
         return (int)e;
     }
     static Kernels get()
@@ -227,6 +229,7 @@ struct xy_state {
     float *theta() const { return reinterpret_cast<float *>(ws + lay.theta); }
     void *labels() const { return ws + lay.labels; }
     uint8_t *bonds() const { return reinterpret_cast<uint8_t *>(ws + lay.bonds); }
+    uint32_t *rootmask() const { return reinterpret_cast<uint32_t *>(ws + lay.rootmask); }
     double *partials() const { return reinterpret_cast<double *>(ws + lay.partials); }
     xy_obs *ring() const { return reinterpret_cast<xy_obs *>(ws + lay.ring); }
     DevCtl *ctl() const { return reinterpret_cast<DevCtl *>(ws + lay.ctl); }
@@ -256,6 +259,7 @@ SweepArgs base_args(const xy_state *s)
     a.theta = s->theta();
     a.labels = s->labels();
     a.bonds = s->bonds();
+    a.rootmask = s->rootmask();
     a.partials = s->partials();
     a.ctl = s->ctl();
     a.ring = s->ring();
@@ -263,6 +267,15 @@ SweepArgs base_args(const xy_state *s)
     a.L = s->L;
     a.tiles_x = s->L / s->ker.tw;
     a.ntiles = a.tiles_x * (s->L / s->ker.th);
+    {
+        // d / L for d < 2^22 (k_flip): with 2^sh <= L < 2^(sh+1), M = ceil(2^(31+sh) / L) <= 2^31 and
+        // floor(d M / 2^(31+sh)) = floor(d / L) because the excess d e / 2^(31+sh) < 2^(-9-sh) < 1/L
+        uint32_t sh = 0;
+        while ((2u << sh) <= s->L) ++sh;
+        const uint64_t num = 1ull << (31 + sh);
+        a.Ldiv_mul = (uint32_t)((num + s->L - 1) / s->L);
+        a.Ldiv_shift = sh - 1;
+    }
     a.seed_lo = (uint32_t)(s->seed & 0xffffffffu);
     a.seed_hi = (uint32_t)(s->seed >> 32);
     a.t = (uint32_t)s->T;

@@ -49,12 +49,14 @@ struct SweepArgs {
     float       *theta;
     void        *labels;
     uint8_t     *bonds;
+    uint32_t    *rootmask;        // 1 bit per site: the site is the root of its tile-local component (k_label -> k_flip)
     double      *partials;        // [grid][kPartialStride]
     DevCtl      *ctl;
     xy_obs      *ring;
     uint32_t     ring_cap;
     uint32_t     L;
     uint32_t     tiles_x, ntiles;
+    uint32_t     Ldiv_mul, Ldiv_shift;   // d / L for d < 2^22: umulhi(d, Ldiv_mul) >> Ldiv_shift
     uint32_t     seed_lo, seed_hi;
     uint32_t     t;               // sweep counter of THIS sweep (state before it has T = t sweeps done)
     int          beta_from_ctl;   // 1: read beta from ctl->beta (PCC), 0: use beta
@@ -371,174 +373,165 @@ k_bonds(const SweepArgs a)
 }
 
 // ---------------------------------------------------------------------------------------------
-// k_label (S3): tile-local labeling from the packed bond bits; integer only.  One CTA per
-// TW x TH tile (TW = 32*VEC, TH = R*NW); warp w owns the strip of rows [w*R, (w+1)*R).
-//   scan   each warp walks its strip top to bottom, all lanes on the same row: run starts of the
-//          row by ballot/clz over the x bits -> parent[]; then every y bond that is not redundant
-//          ATTACHES the lower run's fresh root to the upper site's root, which the lane carries
-//          in registers: one atomicMin, no find.  Only when the run was already attached
-//          elsewhere (two upper components meet) a real union runs.  Row order keeps trees flat.
-//   stitch unions across the NW-1 strip boundaries (generic lock-step union).
-//   emit   provisional label = global index of the tile-local root (min index in the tile-local
-//          component).  Bonds that leave the tile are left to k_merge.
+// k_label (S3): tile-local labeling from the packed bond bits; integer only, bit-parallel.
+// One CTA per TW x TH tile, TW = 32*WPR; thread (r, w) owns WORD w of row r: 32 sites whose x and
+// y bond bits sit in one register each.  The union-find runs over RUNS (maximal chains of x
+// bonds inside the tile); a run is named by the tile-local index of its first site.
+//   prep    X, Y words from the nibble-packed bytes; S = run-start bits; LL = last run start to
+//           the left of the word (runs may span words).
+//   union   every y bond that is not redundant (its left neighbour is joined to it in both rows
+//           and has its own y bond) unites the runs above and below: lock-free min-link union in
+//           shared memory, all rows at once.
+//   flatten every run start finds its root and stores it; a bit per site says "tile-local root"
+//           (rootmask, read by k_flip).
+//   emit    label of a site = global index of the root of its run, 4 sites per thread, coalesced.
+// Bonds that leave the tile are left to k_merge.
 // ---------------------------------------------------------------------------------------------
-template <int VEC, int R, int NW>
-constexpr size_t k_label_smem_bytes() { return (size_t)(32 * VEC) * (R * NW) * 4 + (size_t)NW * 64; }
+template <int WPR, int TH>
+constexpr size_t k_label_smem_bytes() { return (size_t)(32 * WPR) * TH * 4 + (size_t)TH * WPR * 12; }
 
-template <int VEC, int R, int NW, typename LabelT>
-__global__ void __launch_bounds__(NW * 32)
+__device__ __forceinline__ uint32_t nib_lo16(uint32_t v)      // low nibbles of 4 bytes -> 16 bits
+{
+    uint32_t t = v & 0x0F0F0F0Fu;
+    t = (t | (t >> 4)) & 0x00FF00FFu;
+    return (t | (t >> 8)) & 0xFFFFu;
+}
+
+__device__ __forceinline__ uint32_t sfind_v(const volatile uint32_t *p, uint32_t a)
+{
+    uint32_t r = p[a];
+    while (r != a) { a = r; r = p[a]; }
+    return a;
+}
+
+// min-link union of the components of a and b (any nodes)
+__device__ __forceinline__ void sunion_v(uint32_t *p, uint32_t a, uint32_t b)
+{
+    const volatile uint32_t *vp = p;
+    for (;;) {
+        a = sfind_v(vp, a);
+        b = sfind_v(vp, b);
+        if (a == b) return;
+        const uint32_t hi = a > b ? a : b, lo = a > b ? b : a;
+        const uint32_t old = atomicMin(&p[hi], lo);
+        if (old == hi) return;
+        a = old;                                   // hi was linked meanwhile: go on from its new parent
+        b = lo;
+    }
+}
+
+template <int WPR, int TH, typename LabelT>
+__global__ void __launch_bounds__(WPR * TH)
 k_label(const SweepArgs a)
 {
-    constexpr int TW = 32 * VEC, TH = R * NW;
-    constexpr uint32_t VMASK = (1u << VEC) - 1u;
+    constexpr int TW = 32 * WPR, NT = WPR * TH;
+    constexpr uint32_t NONE = 0xffffffffu;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    uint32_t *parent = reinterpret_cast<uint32_t *>(smem_raw);                     // [TW*TH]
-    uint8_t (*xfirst)[32] = reinterpret_cast<uint8_t (*)[32]>(smem_raw + TW * TH * 4);          // x bits of each strip's first row
-    uint8_t (*xlast)[32] = reinterpret_cast<uint8_t (*)[32]>(smem_raw + TW * TH * 4 + NW * 32); // x | y << 4 bits of its last row
+    uint32_t *parent = reinterpret_cast<uint32_t *>(smem_raw);                       // [TW*TH]
+    uint32_t (*Xs)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 4);
+    uint32_t (*Ss)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 4);
+    uint32_t (*LLs)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 8);
 
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t L = a.L;
     LabelT *labels = reinterpret_cast<LabelT *>(a.labels);
     const uint32_t tile = blockIdx.x;
     const uint32_t ty = tile / a.tiles_x, tx = tile - ty * a.tiles_x;
     const uint32_t x0 = tx * TW, y0 = ty * TH;
-    const uint32_t xl = x0 + lane * VEC;
+    const int tid = threadIdx.x;
+    const int r = tid / WPR, w = tid % WPR;
+    const uint32_t base = r * TW + 32 * w;          // tile-local index of this word's first site
 
-    uint32_t bytes[R];
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        uint32_t b = a.bonds[((size_t)(y0 + warp * R + r) * L + xl) >> 2];
-        if constexpr (VEC == 2) b = (b >> ((lane & 1) * 2)) & 0x33u;
-        bytes[r] = b;
+    // ---- prep ----
+    uint32_t X, Y;
+    {
+        const size_t i = (size_t)(y0 + r) * L + x0 + 32 * w;
+        const uint2 raw = __ldg(reinterpret_cast<const uint2 *>(a.bonds + (i >> 2)));
+        X = nib_lo16(raw.x) | (nib_lo16(raw.y) << 16);
+        Y = nib_lo16(raw.x >> 4) | (nib_lo16(raw.y >> 4) << 16);
     }
-
-    // ---- scan ----
-    uint32_t rootU[VEC];            // root (as of the previous row) of the VEC sites above
-    uint32_t xprev = 0, yprev = 0;  // tile-local x bits and y bits of the previous row
+    if (w == WPR - 1) X &= 0x7fffffffu;             // that bond leaves the tile
+    if (r == TH - 1) Y = 0u;                        // so do these
+    const uint32_t xl = __shfl_up_sync(0xffffffffu, X, 1);
+    const uint32_t S = ~((X << 1) | (w > 0 ? xl >> 31 : 0u));
+    const uint32_t lastS = S ? base + 31 - __clz(S) : NONE;
+    uint32_t LL = NONE;
 #pragma unroll
-    for (int v = 0; v < VEC; ++v) rootU[v] = 0;
-#pragma unroll 1
-    for (int r = 0; r < R; ++r) {
-        const int ly = warp * R + r;
-        uint32_t xloc = bytes[0] & VMASK;
-        const uint32_t yn = (bytes[0] >> 4) & VMASK;
-#pragma unroll
-        for (int k = 0; k + 1 < R; ++k) bytes[k] = bytes[k + 1];                 // rotate (keeps indices static)
-        if (lane == 31) xloc &= ~(1u << (VEC - 1));                              // that bond leaves the tile
-        if (r == 0) xfirst[warp][lane] = (uint8_t)xloc;
-        // run starts of this row
-        const uint32_t through = __ballot_sync(0xffffffffu, xloc == VMASK);
-        const uint32_t stop = ~through & ((1u << lane) - 1u);                    // lanes below me that break the run
-        const int lp = stop ? 31 - __clz(stop) : 0;
-        const uint32_t nib = __shfl_sync(0xffffffffu, xloc, lp);
-        uint32_t s0 = 0;
-        if (stop) s0 = lp * VEC + (31 - __clz(~nib & VMASK)) + 1;
-        uint32_t start[VEC];
-        start[0] = ly * TW + s0;
-#pragma unroll
-        for (int v = 1; v < VEC; ++v)
-            start[v] = ((xloc >> (v - 1)) & 1u) ? start[v - 1] : (uint32_t)(ly * TW + lane * VEC + v);
-        if constexpr (VEC == 4)
-            *reinterpret_cast<uint4 *>(&parent[ly * TW + lane * 4]) = make_uint4(start[0], start[1], start[2], start[3]);
-        else
-            *reinterpret_cast<uint2 *>(&parent[ly * TW + lane * 2]) = make_uint2(start[0], start[1]);
-        __syncwarp();
-        if (r > 0) {
-            // a y bond is redundant if the left neighbour is joined to me in both rows and has its own y bond
-            uint32_t dup = (xprev & xloc & yprev) << 1;
-            const uint32_t packed = xprev & xloc & yprev;
-            const uint32_t left = __shfl_up_sync(0xffffffffu, packed, 1);
-            if (lane > 0) dup |= (left >> (VEC - 1)) & 1u;
-            const uint32_t need = yprev & ~dup & VMASK;
-            // attach: the lower run's root takes the upper root unless it already has a smaller one
-            uint32_t fail = 0, other[VEC];
-#pragma unroll
-            for (int v = 0; v < VEC; ++v) {
-                other[v] = 0;
-                if ((need >> v) & 1u) {
-                    const uint32_t old = atomicMin(&parent[start[v]], rootU[v]);
-                    if (old != start[v] && old != rootU[v]) { fail |= 1u << v; other[v] = old; }
-                }
-            }
-            // two upper components met in one lower run: real union (rare)
-            if (__any_sync(0xffffffffu, fail != 0)) {
-#pragma unroll
-                for (int v = 0; v < VEC; ++v)
-                    if ((fail >> v) & 1u) sunion(parent, other[v], rootU[v]);
-            }
-            __syncwarp();
-        }
-        // roots of this row's sites for the next row (one extra hop against staleness)
-#pragma unroll
-        for (int v = 0; v < VEC; ++v) {
-            const uint32_t p1 = (v > 0 && start[v] == start[v - 1]) ? rootU[v - 1] : parent[parent[start[v]]];
-            rootU[v] = p1;
-        }
-        xprev = xloc;
-        yprev = yn;
+    for (int d = 1; d < WPR; ++d) {
+        const uint32_t v = __shfl_up_sync(0xffffffffu, lastS, d);
+        if (LL == NONE && d <= w) LL = v;
     }
-
-    // ---- stitch: strip boundaries IN ORDER, by one warp.  When boundary w is processed the strips
-    //      0..w are already one forest whose roots are final for those strips, so every root of
-    //      strip w+1 links straight to a final root: chains stay site -> run start -> strip root -> root.
-    xlast[warp][lane] = (uint8_t)(xprev | (yprev << 4));
+    Xs[r][w] = X; Ss[r][w] = S; LLs[r][w] = LL;
+#pragma unroll
+    for (int k = 0; k < 8; ++k)
+        *reinterpret_cast<uint4 *>(&parent[base + 4 * k]) =
+            make_uint4(base + 4 * k, base + 4 * k + 1, base + 4 * k + 2, base + 4 * k + 3);
     __syncthreads();
-    if (warp == 0) {
-#pragma unroll 1
-        for (int w = 0; w + 1 < NW; ++w) {
-            const uint32_t bu = xlast[w][lane], xu = bu & VMASK, yu = bu >> 4;
-            const uint32_t xd = xfirst[w + 1][lane];
-            const uint32_t packed = xu & xd & yu;
-            uint32_t dup = packed << 1;
-            const uint32_t left = __shfl_up_sync(0xffffffffu, packed, 1);
-            if (lane > 0) dup |= (left >> (VEC - 1)) & 1u;
-            const uint32_t need = yu & ~dup & VMASK;
-            const uint32_t above = (w * R + R - 1) * TW + lane * VEC;
-#pragma unroll
-            for (int v = 0; v < VEC; ++v)
-                if ((need >> v) & 1u) sunion(parent, parent[above + v], parent[above + TW + v]);
-            __syncwarp();
+
+    // ---- union ----
+    {
+        const int rb = (r + 1 < TH) ? r + 1 : r;
+        const uint32_t Xb = Xs[rb][w], Sb = Ss[rb][w], LLb = LLs[rb][w];
+        const uint32_t J = X & Xb & Y;
+        const uint32_t jl = __shfl_up_sync(0xffffffffu, J, 1);
+        uint32_t need = Y & ~((J << 1) | (w > 0 ? jl >> 31 : 0u));
+        while (need) {
+            const int c = __ffs(need) - 1;
+            need &= need - 1;
+            const uint32_t m = (2u << c) - 1u;                                     // bits <= c
+            const uint32_t mt = S & m, mb = Sb & m;
+            const uint32_t at = mt ? base + 31 - __clz(mt) : LL;
+            const uint32_t ab = mb ? base + TW + 31 - __clz(mb) : LLb;
+            sunion_v(parent, at, ab);
         }
     }
     __syncthreads();
 
-    // ---- emit: provisional labels (three hops unrolled for all VEC sites, then the rare rest) ----
-#pragma unroll
-    for (int r = 0; r < R; ++r) {
-        const int ly = warp * R + r;
-        uint32_t p0[VEC], p1[VEC];
-        if constexpr (VEC == 4) {
-            const uint4 q = *reinterpret_cast<const uint4 *>(&parent[ly * TW + lane * 4]);
-            p0[0] = q.x; p0[1] = q.y; p0[2] = q.z; p0[3] = q.w;
-        } else {
-            const uint2 q = *reinterpret_cast<const uint2 *>(&parent[ly * TW + lane * 2]);
-            p0[0] = q.x; p0[1] = q.y;
+    // ---- flatten the run starts; which sites are tile-local roots ----
+    {
+        uint32_t rootbits = 0, rem = S;
+        const volatile uint32_t *vp = parent;
+        while (rem) {
+            const int c = __ffs(rem) - 1;
+            rem &= rem - 1;
+            const uint32_t s = base + c;
+            const uint32_t root = sfind_v(vp, s);
+            if (root != s) parent[s] = root;        // readers in flight see an ancestor either way
+            else rootbits |= 1u << c;
         }
+        a.rootmask[((size_t)(y0 + r) * L + x0 + 32 * w) >> 5] = rootbits;
+    }
+    __syncthreads();
+
+    // ---- emit: 4 consecutive sites per thread, one row per (TW/4) threads ----
+    constexpr int Q = TW / 4, RPP = NT / Q;          // quads per row, rows per pass
+    const int q = tid % Q, rq = tid / Q;
+    const int wq = q >> 3, o = (q & 7) * 4;
+    const LabelT gbase = (LabelT)y0 * L + x0;
+#pragma unroll 2
+    for (int k = 0; k < TH / RPP; ++k) {
+        const int row = k * RPP + rq;
+        const uint32_t Sq = Ss[row][wq];
+        const uint32_t wbase = row * TW + 32 * wq;
+        const uint32_t m = Sq & ((2u << o) - 1u);
+        uint32_t st = m ? wbase + 31 - __clz(m) : LLs[row][wq];
+        uint32_t root = parent[st];
+        LabelT out[4];
+        out[0] = gbase + (LabelT)(root / TW) * L + (root % TW);
 #pragma unroll
-        for (int v = 0; v < VEC; ++v) p1[v] = parent[p0[v]];
-#pragma unroll
-        for (int v = 0; v < VEC; ++v) p0[v] = parent[p1[v]];
-#pragma unroll
-        for (int v = 0; v < VEC; ++v) p1[v] = parent[p0[v]];
-        // now p0 = 2 hops above the site's run start, p1 = parent[p0]
-#pragma unroll
-        for (int v = 0; v < VEC; ++v) { const uint32_t t = p0[v]; p0[v] = p1[v]; p1[v] = t; }
-        LabelT out[VEC];
-#pragma unroll
-        for (int v = 0; v < VEC; ++v) {
-            uint32_t root = p0[v];
-            if (root != p1[v]) root = sfind(parent, root);
-            const uint32_t ry = root / TW, rx = root - ry * TW;
-            out[v] = (LabelT)(y0 + ry) * L + (x0 + rx);
+        for (int v = 1; v < 4; ++v) {
+            if ((Sq >> (o + v)) & 1u) {
+                root = parent[wbase + o + v];
+                out[v] = gbase + (LabelT)(root / TW) * L + (root % TW);
+            } else {
+                out[v] = out[v - 1];
+            }
         }
-        LabelT *dst = labels + (size_t)(y0 + ly) * L + xl;
+        LabelT *dst = labels + (size_t)(y0 + row) * L + x0 + 4 * q;
         if constexpr (sizeof(LabelT) == 4) {
-            if constexpr (VEC == 4) *reinterpret_cast<uint4 *>(dst) = make_uint4(out[0], out[1], out[2], out[3]);
-            else *reinterpret_cast<uint2 *>(dst) = make_uint2(out[0], out[1]);
+            *reinterpret_cast<uint4 *>(dst) = make_uint4(out[0], out[1], out[2], out[3]);
         } else {
-#pragma unroll
-            for (int v = 0; v < VEC; v += 2)
-                *reinterpret_cast<ulonglong2 *>(dst + v) = make_ulonglong2(out[v], out[v + 1]);
+            *reinterpret_cast<ulonglong2 *>(dst) = make_ulonglong2(out[0], out[1]);
+            *reinterpret_cast<ulonglong2 *>(dst + 2) = make_ulonglong2(out[2], out[3]);
         }
     }
 }
@@ -577,84 +570,136 @@ k_merge(const SweepArgs a)
 }
 
 // ---------------------------------------------------------------------------------------------
-// k_flip: root of every site (read-only chase; the forest is final after k_merge), coin of the
-// root, reflection.  One CTA per TW x TH tile so that the first hop of every chase (the tile-local
-// root) is served by L1.  Counts the clusters (#{root == site}).
+// k_flip (S5 + S6): coin of every site's cluster, reflection, cluster count.  One CTA per
+// TW x TH tile (the tiles of k_label), 4 consecutive sites x TH/RPP rows per thread.
+//   coins   one Philox call per tile row gives the coins of all 128 labels of that row
+//           (coin of label rho = bit rho mod 128 of the call keyed by rho div 128).
+//   roots   a tile-local root that still is a global root (label == own index) takes its coin
+//           from that table; one that k_merge linked elsewhere is queued, and the queue is
+//           worked off densely: chase to the global root (read-only: the forest is final),
+//           one Philox call for that root.  Each tile root publishes its coin in shared memory.
+//   sites   every other site reads the coin published by its tile root (its label), reflects,
+//           and rows in which nothing flipped are not written back.
 // ---------------------------------------------------------------------------------------------
-template <int VEC, int R, int NW, typename LabelT>
-__global__ void __launch_bounds__(NW * 32)
+template <int WPR, int TH, typename LabelT>
+__global__ void __launch_bounds__(WPR * TH)
 k_flip(const SweepArgs a)
 {
-    constexpr int TW = 32 * VEC, TH = R * NW;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    constexpr int TW = 32 * WPR, NT = WPR * TH;
+    constexpr int Q = TW / 4, RPP = NT / Q, NP = TH / RPP;
+    __shared__ uint32_t coinrow[TH][4];
+    __shared__ uint8_t cb[TW * TH];
+    __shared__ uint32_t queue[2 * (TW + TH)];        // merged tile roots: each owns a component that touches the tile edge, so at most one per edge site
+    __shared__ uint32_t nqueue;
+    __shared__ unsigned long long sc[NT / 32];
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t L = a.L;
     const LabelT *labels = reinterpret_cast<const LabelT *>(a.labels);
-    uint32_t ncl = 0;
-    for (uint32_t tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
-        const uint32_t ty = tile / a.tiles_x, tx = tile - ty * a.tiles_x;
-        const uint32_t xl = tx * TW + lane * VEC;
-        const uint32_t yb = ty * TH + warp * R;
-        LabelT lab[R][VEC];
-        float th[R][VEC];
+    const uint32_t tile = blockIdx.x;
+    const uint32_t ty = tile / a.tiles_x, tx = tile - ty * a.tiles_x;
+    const uint32_t x0 = tx * TW, y0 = ty * TH;
+    const int q = tid % Q, rq = tid / Q;
+    const LabelT gbase = (LabelT)y0 * L + x0;
+
+    if (tid == 0) nqueue = 0;
+    if (tid < TH) {
+        const uint64_t g = (uint64_t)(y0 + tid) * L + x0;
+        const U4 c = rng(a.seed_lo, a.seed_hi, g >> 7, a.t, TAG_FLIP);
+        if (TW == 128 || (g & 64u) == 0) { coinrow[tid][0] = c.x; coinrow[tid][1] = c.y; coinrow[tid][2] = c.z; coinrow[tid][3] = c.w; }
+        else { coinrow[tid][0] = c.z; coinrow[tid][1] = c.w; coinrow[tid][2] = 0; coinrow[tid][3] = 0; }
+    }
+
+    LabelT lab[NP][4];
+    float th[NP][4];
+    uint32_t rb[NP];
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const size_t i = (size_t)(yb + r) * L + xl;
-            if constexpr (sizeof(LabelT) == 4) {
-                if constexpr (VEC == 4) {
-                    const uint4 v = __ldg(reinterpret_cast<const uint4 *>(labels + i));
-                    lab[r][0] = v.x; lab[r][1] = v.y; lab[r][2] = v.z; lab[r][3] = v.w;
-                } else {
-                    const uint2 v = __ldg(reinterpret_cast<const uint2 *>(labels + i));
-                    lab[r][0] = v.x; lab[r][1] = v.y;
-                }
-            } else {
-#pragma unroll
-                for (int v = 0; v < VEC; v += 2) {
-                    const ulonglong2 q = __ldg(reinterpret_cast<const ulonglong2 *>(labels + i + v));
-                    lab[r][v] = q.x; lab[r][v + 1] = q.y;
-                }
-            }
-            load_vec<VEC, false>(a.theta + i, th[r]);
+    for (int k = 0; k < NP; ++k) {
+        const int row = k * RPP + rq;
+        const size_t i = (size_t)(y0 + row) * L + x0 + 4 * q;
+        if constexpr (sizeof(LabelT) == 4) {
+            const uint4 v = __ldg(reinterpret_cast<const uint4 *>(labels + i));
+            lab[k][0] = v.x; lab[k][1] = v.y; lab[k][2] = v.z; lab[k][3] = v.w;
+        } else {
+            const ulonglong2 u = __ldg(reinterpret_cast<const ulonglong2 *>(labels + i));
+            const ulonglong2 v = __ldg(reinterpret_cast<const ulonglong2 *>(labels + i + 2));
+            lab[k][0] = u.x; lab[k][1] = u.y; lab[k][2] = v.x; lab[k][3] = v.y;
         }
+        const float4 t = *reinterpret_cast<const float4 *>(a.theta + i);
+        th[k][0] = t.x; th[k][1] = t.y; th[k][2] = t.z; th[k][3] = t.w;
+        rb[k] = (__ldg(reinterpret_cast<const uint8_t *>(a.rootmask) + (i >> 3)) >> (i & 4u)) & 15u;
+    }
+    __syncthreads();
+
+    // ---- tile roots publish their coin ----
+    uint32_t ncl = 0;
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const size_t i = (size_t)(yb + r) * L + xl;
-            LabelT prev_l = (LabelT)~(LabelT)0, prev_root = 0;
-            bool prev_coin = false, any = false;
-            float out[VEC];
+    for (int k = 0; k < NP; ++k) {
+        if (rb[k]) {
+            const int row = k * RPP + rq;
+            const uint32_t loc0 = row * TW + 4 * q;
+            const uint32_t cw = coinrow[row][q >> 3] >> ((q & 7) * 4);
 #pragma unroll
-            for (int v = 0; v < VEC; ++v) {
-                const LabelT l0 = lab[r][v];
-                LabelT root;
-                bool coin;
-                if (v > 0 && l0 == prev_l) {
-                    root = prev_root; coin = prev_coin;
-                } else {
-                    root = l0;
-                    if (l0 != (LabelT)(i + v)) {
-                        LabelT p = __ldg(labels + root);
-                        while (p != root) { root = p; p = __ldg(labels + root); }
+            for (int v = 0; v < 4; ++v) {
+                if ((rb[k] >> v) & 1u) {
+                    if (lab[k][v] == gbase + (LabelT)row * L + (4 * q + v)) {
+                        cb[loc0 + v] = (uint8_t)((cw >> v) & 1u);
+                        ++ncl;
+                    } else {
+                        queue[atomicAdd(&nqueue, 1u)] = loc0 + v;
                     }
-                    coin = (rng(a.seed_lo, a.seed_hi, (uint64_t)root, a.t, TAG_FLIP).x >> 31) != 0u;
                 }
-                prev_l = l0; prev_root = root; prev_coin = coin;
-                ncl += (root == (LabelT)(i + v));
-                out[v] = coin ? reflect(th[r][v], a.A) : th[r][v];
-                any |= coin;
-            }
-            if (any) {
-                if constexpr (VEC == 4) *reinterpret_cast<float4 *>(a.theta + i) = make_float4(out[0], out[1], out[2], out[3]);
-                else *reinterpret_cast<float2 *>(a.theta + i) = make_float2(out[0], out[1]);
             }
         }
     }
+    __syncthreads();
+    {
+        const uint32_t nq = nqueue;
+        for (uint32_t j = tid; j < nq; j += NT) {
+            const uint32_t loc = queue[j];
+            LabelT root = __ldg(labels + gbase + (LabelT)(loc / TW) * L + (loc % TW));
+            LabelT p = __ldg(labels + root);
+            while (p != root) { root = p; p = __ldg(labels + root); }
+            const U4 c = rng(a.seed_lo, a.seed_hi, (uint64_t)root >> 7, a.t, TAG_FLIP);
+            const uint32_t sel = ((uint32_t)root >> 5) & 3u;
+            const uint32_t word = sel == 0 ? c.x : sel == 1 ? c.y : sel == 2 ? c.z : c.w;
+            cb[loc] = (uint8_t)((word >> ((uint32_t)root & 31u)) & 1u);
+        }
+    }
+    __syncthreads();
+
+    // ---- every site takes the coin of its tile root; reflect ----
+    const uint32_t Lm = L - TW;
+#pragma unroll
+    for (int k = 0; k < NP; ++k) {
+        const int row = k * RPP + rq;
+        const uint32_t loc0 = row * TW + 4 * q;
+        float out[4];
+        bool any = false;
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+            uint32_t loc = loc0 + v;
+            if (!((rb[k] >> v) & 1u)) {
+                const uint32_t d = (uint32_t)(lab[k][v] - gbase);          // r*L + c, < TH*L <= 2^22
+                const uint32_t rr = __umulhi(d, a.Ldiv_mul) >> a.Ldiv_shift;
+                loc = d - rr * Lm;
+            }
+            const bool coin = cb[loc] != 0;
+            out[v] = coin ? reflect(th[k][v], a.A) : th[k][v];
+            any |= coin;
+        }
+        if (any) {
+            const size_t i = (size_t)(y0 + row) * L + x0 + 4 * q;
+            *reinterpret_cast<float4 *>(a.theta + i) = make_float4(out[0], out[1], out[2], out[3]);
+        }
+    }
+
     unsigned long long c = warp_sum_u64(ncl);
-    __shared__ unsigned long long sc[NW];
     if (lane == 0) sc[warp] = c;
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (tid == 0) {
         unsigned long long tot = 0;
-        for (int w = 0; w < NW; ++w) tot += sc[w];
+        for (int w = 0; w < NT / 32; ++w) tot += sc[w];
         xy_obs *o = a.ring + ((a.t + 1u) % a.ring_cap);
         atomicAdd(reinterpret_cast<unsigned long long *>(&o->n_clusters), tot);
     }

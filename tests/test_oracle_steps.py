@@ -276,8 +276,15 @@ def test_flip_is_per_cluster_and_fair():
     # fair coin over many clusters
     coins = np.array([xo.flip_coin(seed, r, tt) for r in range(2000) for tt in range(10)])
     assert abs(coins.mean() - 0.5) < 4 * 0.5 / math.sqrt(coins.size)
-    w = xo.rng(seed, 1234, t, xo.TAG_FLIP)
-    assert xo.flip_coin(seed, 1234, t) == int(w[0]) >> 31
+    # one Philox call serves 128 consecutive labels: coin = bit (rho mod 128) of its 128-bit output
+    for rho in (0, 1, 31, 32, 127, 128, 1234, 2**32 - 1, 2**32 + 77):
+        w = xo.rng(seed, rho >> 7, t, xo.TAG_FLIP)
+        assert xo.flip_coin(seed, rho, t) == (int(w[(rho >> 5) & 3]) >> (rho & 31)) & 1
+    # neighbouring labels (same Philox call) are uncorrelated
+    c = np.array([xo.flip_coin(seed, r, t) for r in range(1 << 14)], dtype=np.float64) - 0.5
+    for lag in (1, 2, 32, 64, 127, 128):
+        corr = 4.0 * (c[:-lag] * c[lag:]).mean()
+        assert abs(corr) < 4.0 / math.sqrt(c.size - lag)
 
 
 # ------------------------------------------------------------------ observables (O7)
