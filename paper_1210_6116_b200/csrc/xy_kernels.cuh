@@ -404,13 +404,28 @@ __device__ __forceinline__ uint32_t sfind_v(const volatile uint32_t *p, uint32_t
     return a;
 }
 
+// find with path halving: every node on the way is re-pointed to its grandparent.  Racing writers
+// only ever replace a parent by an ancestor, so concurrent finds and min-links stay correct.
+__device__ __forceinline__ uint32_t sfind_h(volatile uint32_t *p, uint32_t a)
+{
+    uint32_t r = p[a];
+    while (r != a) {
+        const uint32_t g = p[r];
+        if (g == r) return r;
+        p[a] = g;
+        a = g;
+        r = p[a];
+    }
+    return a;
+}
+
 // min-link union of the components of a and b (any nodes)
 __device__ __forceinline__ void sunion_v(uint32_t *p, uint32_t a, uint32_t b)
 {
-    const volatile uint32_t *vp = p;
+    volatile uint32_t *vp = p;
     for (;;) {
-        a = sfind_v(vp, a);
-        b = sfind_v(vp, b);
+        a = sfind_h(vp, a);
+        b = sfind_h(vp, b);
         if (a == b) return;
         const uint32_t hi = a > b ? a : b, lo = a > b ? b : a;
         const uint32_t old = atomicMin(&p[hi], lo);
@@ -421,7 +436,7 @@ __device__ __forceinline__ void sunion_v(uint32_t *p, uint32_t a, uint32_t b)
 }
 
 template <int WPR, int TH, typename LabelT>
-__global__ void __launch_bounds__(WPR * TH)
+__global__ void __launch_bounds__(WPR * TH, 1536 / (WPR * TH))
 k_label(const SweepArgs a)
 {
     constexpr int TW = 32 * WPR, NT = WPR * TH;
@@ -582,13 +597,12 @@ k_merge(const SweepArgs a)
 //           and rows in which nothing flipped are not written back.
 // ---------------------------------------------------------------------------------------------
 template <int WPR, int TH, typename LabelT>
-__global__ void __launch_bounds__(WPR * TH)
+__global__ void __launch_bounds__(WPR * TH, (sizeof(LabelT) == 4 ? 768 : 512) / (WPR * TH))
 k_flip(const SweepArgs a)
 {
     constexpr int TW = 32 * WPR, NT = WPR * TH;
     constexpr int Q = TW / 4, RPP = NT / Q, NP = TH / RPP;
-    __shared__ uint32_t coinrow[TH][4];
-    __shared__ uint8_t cb[TW * TH];
+    __shared__ uint32_t cbits[TH * WPR];             // coin of the tile root at tile-local index loc: bit loc
     __shared__ uint32_t queue[2 * (TW + TH)];        // merged tile roots: each owns a component that touches the tile edge, so at most one per edge site
     __shared__ uint32_t nqueue;
     __shared__ unsigned long long sc[NT / 32];
@@ -606,13 +620,17 @@ k_flip(const SweepArgs a)
     if (tid < TH) {
         const uint64_t g = (uint64_t)(y0 + tid) * L + x0;
         const U4 c = rng(a.seed_lo, a.seed_hi, g >> 7, a.t, TAG_FLIP);
-        if (TW == 128 || (g & 64u) == 0) { coinrow[tid][0] = c.x; coinrow[tid][1] = c.y; coinrow[tid][2] = c.z; coinrow[tid][3] = c.w; }
-        else { coinrow[tid][0] = c.z; coinrow[tid][1] = c.w; coinrow[tid][2] = 0; coinrow[tid][3] = 0; }
+        if constexpr (WPR == 4) {
+            *reinterpret_cast<uint4 *>(&cbits[tid * 4]) = make_uint4(c.x, c.y, c.z, c.w);
+        } else {
+            const bool up = (g & 64u) != 0;
+            cbits[tid * 2] = up ? c.z : c.x;
+            cbits[tid * 2 + 1] = up ? c.w : c.y;
+        }
     }
 
     LabelT lab[NP][4];
-    float th[NP][4];
-    uint32_t rb[NP];
+    uint32_t rb = 0;                                 // root bits of my 4 sites in pass k: nibble k
 #pragma unroll
     for (int k = 0; k < NP; ++k) {
         const int row = k * RPP + rq;
@@ -625,32 +643,26 @@ k_flip(const SweepArgs a)
             const ulonglong2 v = __ldg(reinterpret_cast<const ulonglong2 *>(labels + i + 2));
             lab[k][0] = u.x; lab[k][1] = u.y; lab[k][2] = v.x; lab[k][3] = v.y;
         }
-        const float4 t = *reinterpret_cast<const float4 *>(a.theta + i);
-        th[k][0] = t.x; th[k][1] = t.y; th[k][2] = t.z; th[k][3] = t.w;
-        rb[k] = (__ldg(reinterpret_cast<const uint8_t *>(a.rootmask) + (i >> 3)) >> (i & 4u)) & 15u;
+        const uint32_t nib = (__ldg(reinterpret_cast<const uint8_t *>(a.rootmask) + (i >> 3)) >> (i & 4u)) & 15u;
+        rb |= nib << (4 * k);
     }
-    __syncthreads();
 
-    // ---- tile roots publish their coin ----
-    uint32_t ncl = 0;
+    // ---- tile roots that k_merge linked elsewhere are queued; the others are the clusters ----
+    uint32_t merged = 0;
 #pragma unroll
     for (int k = 0; k < NP; ++k) {
-        if (rb[k]) {
-            const int row = k * RPP + rq;
-            const uint32_t loc0 = row * TW + 4 * q;
-            const uint32_t cw = coinrow[row][q >> 3] >> ((q & 7) * 4);
+        const LabelT own = gbase + (LabelT)(k * RPP + rq) * L + 4 * q;
 #pragma unroll
-            for (int v = 0; v < 4; ++v) {
-                if ((rb[k] >> v) & 1u) {
-                    if (lab[k][v] == gbase + (LabelT)row * L + (4 * q + v)) {
-                        cb[loc0 + v] = (uint8_t)((cw >> v) & 1u);
-                        ++ncl;
-                    } else {
-                        queue[atomicAdd(&nqueue, 1u)] = loc0 + v;
-                    }
-                }
-            }
-        }
+        for (int v = 0; v < 4; ++v)
+            if (lab[k][v] != own + v) merged |= 1u << (4 * k + v);
+    }
+    merged &= rb;
+    const uint32_t ncl = __popc(rb & ~merged);
+    __syncthreads();                                 // nqueue = 0 and cbits visible
+    while (merged) {
+        const int b = __ffs(merged) - 1;
+        merged &= merged - 1;
+        queue[atomicAdd(&nqueue, 1u)] = ((b >> 2) * RPP + rq) * TW + 4 * q + (b & 3);
     }
     __syncthreads();
     {
@@ -663,7 +675,9 @@ k_flip(const SweepArgs a)
             const U4 c = rng(a.seed_lo, a.seed_hi, (uint64_t)root >> 7, a.t, TAG_FLIP);
             const uint32_t sel = ((uint32_t)root >> 5) & 3u;
             const uint32_t word = sel == 0 ? c.x : sel == 1 ? c.y : sel == 2 ? c.z : c.w;
-            cb[loc] = (uint8_t)((word >> ((uint32_t)root & 31u)) & 1u);
+            const uint32_t coin = (word >> ((uint32_t)root & 31u)) & 1u;
+            if (coin) atomicOr(&cbits[loc >> 5], 1u << (loc & 31u));
+            else atomicAnd(&cbits[loc >> 5], ~(1u << (loc & 31u)));
         }
     }
     __syncthreads();
@@ -674,24 +688,24 @@ k_flip(const SweepArgs a)
     for (int k = 0; k < NP; ++k) {
         const int row = k * RPP + rq;
         const uint32_t loc0 = row * TW + 4 * q;
+        const size_t i = (size_t)(y0 + row) * L + x0 + 4 * q;
+        const float4 t4 = *reinterpret_cast<const float4 *>(a.theta + i);
+        const float th[4] = {t4.x, t4.y, t4.z, t4.w};
         float out[4];
         bool any = false;
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
             uint32_t loc = loc0 + v;
-            if (!((rb[k] >> v) & 1u)) {
+            if (!((rb >> (4 * k + v)) & 1u)) {
                 const uint32_t d = (uint32_t)(lab[k][v] - gbase);          // r*L + c, < TH*L <= 2^22
                 const uint32_t rr = __umulhi(d, a.Ldiv_mul) >> a.Ldiv_shift;
                 loc = d - rr * Lm;
             }
-            const bool coin = cb[loc] != 0;
-            out[v] = coin ? reflect(th[k][v], a.A) : th[k][v];
+            const bool coin = (cbits[loc >> 5] >> (loc & 31u)) & 1u;
+            out[v] = coin ? reflect(th[v], a.A) : th[v];
             any |= coin;
         }
-        if (any) {
-            const size_t i = (size_t)(y0 + row) * L + x0 + 4 * q;
-            *reinterpret_cast<float4 *>(a.theta + i) = make_float4(out[0], out[1], out[2], out[3]);
-        }
+        if (any) *reinterpret_cast<float4 *>(a.theta + i) = make_float4(out[0], out[1], out[2], out[3]);
     }
 
     unsigned long long c = warp_sum_u64(ncl);
