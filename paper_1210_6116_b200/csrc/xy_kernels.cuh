@@ -388,7 +388,7 @@ k_bonds(const SweepArgs a)
 // Bonds that leave the tile are left to k_merge.
 // ---------------------------------------------------------------------------------------------
 template <int WPR, int TH>
-constexpr size_t k_label_smem_bytes() { return (size_t)(32 * WPR) * TH * 4 + (size_t)TH * WPR * 12; }
+constexpr size_t k_label_smem_bytes() { return (size_t)(32 * WPR) * TH * 4 + (size_t)TH * WPR * 16; }
 
 __device__ __forceinline__ uint32_t nib_lo16(uint32_t v)      // low nibbles of 4 bytes -> 16 bits
 {
@@ -446,6 +446,7 @@ k_label(const SweepArgs a)
     uint32_t (*Xs)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 4);
     uint32_t (*Ss)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 4);
     uint32_t (*LLs)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 8);
+    uint32_t (*Ns)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 12);   // y bonds that unite two runs
 
     const uint32_t L = a.L;
     LabelT *labels = reinterpret_cast<LabelT *>(a.labels);
@@ -482,24 +483,44 @@ k_label(const SweepArgs a)
             make_uint4(base + 4 * k, base + 4 * k + 1, base + 4 * k + 2, base + 4 * k + 3);
     __syncthreads();
 
-    // ---- union ----
+    // ---- which y bonds unite two runs: not the redundant ones ----
     {
         const int rb = (r + 1 < TH) ? r + 1 : r;
-        const uint32_t Xb = Xs[rb][w], Sb = Ss[rb][w], LLb = LLs[rb][w];
-        const uint32_t J = X & Xb & Y;
+        const uint32_t J = X & Xs[rb][w] & Y;
         const uint32_t jl = __shfl_up_sync(0xffffffffu, J, 1);
-        uint32_t need = Y & ~((J << 1) | (w > 0 ? jl >> 31 : 0u));
-        while (need) {
-            const int c = __ffs(need) - 1;
-            need &= need - 1;
-            const uint32_t m = (2u << c) - 1u;                                     // bits <= c
-            const uint32_t mt = S & m, mb = Sb & m;
-            const uint32_t at = mt ? base + 31 - __clz(mt) : LL;
-            const uint32_t ab = mb ? base + TW + 31 - __clz(mb) : LLb;
-            sunion_v(parent, at, ab);
-        }
+        Ns[r][w] = Y & ~((J << 1) | (w > 0 ? jl >> 31 : 0u));
     }
     __syncthreads();
+
+    // ---- union, in log2(TH) waves: wave j joins blocks of 2^(j-1) rows pairwise, so every wave
+    //      links roots of forests that are already flat and the trees stay shallow.  The boundary
+    //      rows of a wave are spread over ALL threads (cpi columns each).
+#pragma unroll
+    for (int j = 1; (1 << j) <= TH; ++j) {
+        const int nb = TH >> j;                                // boundaries in this wave
+        const int cpi = (32 >> j) > 0 ? (32 >> j) : 1;         // columns per work item
+        const int ipb = TW / cpi;                              // items per boundary
+        if (tid < nb * ipb) {
+            const int kb = tid / ipb, it = tid - kb * ipb;
+            const int rt = (1 << (j - 1)) - 1 + (kb << j);     // upper row of the boundary
+            const int col0 = it * cpi, ww = col0 >> 5, off = col0 & 31;
+            uint32_t need = Ns[rt][ww] & (((1u << cpi) - 1u) << off);
+            if (need) {
+                const uint32_t St = Ss[rt][ww], Sb = Ss[rt + 1][ww];
+                const uint32_t bt = rt * TW + 32 * ww;
+                do {
+                    const int c = __ffs(need) - 1;
+                    need &= need - 1;
+                    const uint32_t m = (2u << c) - 1u;                             // bits <= c
+                    const uint32_t mt = St & m, mb = Sb & m;
+                    const uint32_t at = mt ? bt + 31 - __clz(mt) : LLs[rt][ww];
+                    const uint32_t ab = mb ? bt + TW + 31 - __clz(mb) : LLs[rt + 1][ww];
+                    sunion_v(parent, at, ab);
+                } while (need);
+            }
+        }
+        __syncthreads();
+    }
 
     // ---- flatten the run starts; which sites are tile-local roots ----
     {
