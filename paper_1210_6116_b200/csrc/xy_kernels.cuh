@@ -477,11 +477,28 @@ k_label(const SweepArgs a)
         if (LL == NONE && d <= w) LL = v;
     }
     Xs[r][w] = X; Ss[r][w] = S; LLs[r][w] = LL;
-#pragma unroll
-    for (int k = 0; k < 8; ++k)
-        *reinterpret_cast<uint4 *>(&parent[base + 4 * k]) =
-            make_uint4(base + 4 * k, base + 4 * k + 1, base + 4 * k + 2, base + 4 * k + 3);
     __syncthreads();
+
+    // quad mapping (4 consecutive sites per thread, one row per TW/4 threads): conflict-free 16-byte
+    // accesses to parent[] and coalesced label stores
+    constexpr int Q = TW / 4, RPP = NT / Q;          // quads per row, rows per pass
+    const int q = tid % Q, rq = tid / Q;
+    const int wq = q >> 3, o = (q & 7) * 4;
+
+    // ---- parent[site] = first site of its run (a run start points to itself) ----
+#pragma unroll 2
+    for (int k = 0; k < TH / RPP; ++k) {
+        const int row = k * RPP + rq;
+        const uint32_t Sq = Ss[row][wq];
+        const uint32_t wbase = row * TW + 32 * wq;
+        const uint32_t m = Sq & ((2u << o) - 1u);
+        uint4 st;
+        st.x = m ? wbase + 31 - __clz(m) : LLs[row][wq];
+        st.y = ((Sq >> (o + 1)) & 1u) ? wbase + o + 1 : st.x;
+        st.z = ((Sq >> (o + 2)) & 1u) ? wbase + o + 2 : st.y;
+        st.w = ((Sq >> (o + 3)) & 1u) ? wbase + o + 3 : st.z;
+        *reinterpret_cast<uint4 *>(&parent[wbase + o]) = st;
+    }
 
     // ---- which y bonds unite two runs: not the redundant ones ----
     {
@@ -522,53 +539,49 @@ k_label(const SweepArgs a)
         __syncthreads();
     }
 
-    // ---- flatten the run starts; which sites are tile-local roots ----
-    {
-        uint32_t rootbits = 0, rem = S;
-        const volatile uint32_t *vp = parent;
-        while (rem) {
-            const int c = __ffs(rem) - 1;
-            rem &= rem - 1;
-            const uint32_t s = base + c;
-            const uint32_t root = sfind_v(vp, s);
-            if (root != s) parent[s] = root;        // readers in flight see an ancestor either way
-            else rootbits |= 1u << c;
+    // ---- flatten by pointer jumping over ALL entries (fixed cost, no divergence): parent[i] <-
+    //      parent[parent[i]] until nothing changes.  In place: a racing reader sees an ancestor.
+    for (;;) {
+        bool changed = false;
+#pragma unroll 2
+        for (int k = 0; k < TH / RPP; ++k) {
+            const uint32_t i0 = (k * RPP + rq) * TW + 4 * q;
+            const uint4 p1 = *reinterpret_cast<const uint4 *>(&parent[i0]);
+            uint4 p2;
+            p2.x = parent[p1.x]; p2.y = parent[p1.y]; p2.z = parent[p1.z]; p2.w = parent[p1.w];
+            if (p2.x != p1.x || p2.y != p1.y || p2.z != p1.z || p2.w != p1.w) {
+                *reinterpret_cast<uint4 *>(&parent[i0]) = p2;
+                changed = true;
+            }
         }
-        a.rootmask[((size_t)(y0 + r) * L + x0 + 32 * w) >> 5] = rootbits;
+        if (!__syncthreads_or(changed)) break;
     }
-    __syncthreads();
 
-    // ---- emit: 4 consecutive sites per thread, one row per (TW/4) threads ----
-    constexpr int Q = TW / 4, RPP = NT / Q;          // quads per row, rows per pass
-    const int q = tid % Q, rq = tid / Q;
-    const int wq = q >> 3, o = (q & 7) * 4;
+    // ---- emit: label = global index of the root; rootmask bit = "I am the tile-local root" ----
     const LabelT gbase = (LabelT)y0 * L + x0;
 #pragma unroll 2
     for (int k = 0; k < TH / RPP; ++k) {
         const int row = k * RPP + rq;
-        const uint32_t Sq = Ss[row][wq];
-        const uint32_t wbase = row * TW + 32 * wq;
-        const uint32_t m = Sq & ((2u << o) - 1u);
-        uint32_t st = m ? wbase + 31 - __clz(m) : LLs[row][wq];
-        uint32_t root = parent[st];
+        const uint32_t i0 = row * TW + 4 * q;
+        const uint4 rt = *reinterpret_cast<const uint4 *>(&parent[i0]);
+        const uint32_t root[4] = {rt.x, rt.y, rt.z, rt.w};
         LabelT out[4];
-        out[0] = gbase + (LabelT)(root / TW) * L + (root % TW);
+        uint32_t nib = 0;
 #pragma unroll
-        for (int v = 1; v < 4; ++v) {
-            if ((Sq >> (o + v)) & 1u) {
-                root = parent[wbase + o + v];
-                out[v] = gbase + (LabelT)(root / TW) * L + (root % TW);
-            } else {
-                out[v] = out[v - 1];
-            }
+        for (int v = 0; v < 4; ++v) {
+            out[v] = gbase + (LabelT)(root[v] / TW) * L + (root[v] % TW);
+            nib |= (root[v] == i0 + v) ? (1u << v) : 0u;
         }
-        LabelT *dst = labels + (size_t)(y0 + row) * L + x0 + 4 * q;
+        const size_t gi = (size_t)(y0 + row) * L + x0 + 4 * q;
+        LabelT *dst = labels + gi;
         if constexpr (sizeof(LabelT) == 4) {
             *reinterpret_cast<uint4 *>(dst) = make_uint4(out[0], out[1], out[2], out[3]);
         } else {
             *reinterpret_cast<ulonglong2 *>(dst) = make_ulonglong2(out[0], out[1]);
             *reinterpret_cast<ulonglong2 *>(dst + 2) = make_ulonglong2(out[2], out[3]);
         }
+        const uint32_t hi = __shfl_down_sync(0xffffffffu, nib, 1);
+        if ((q & 1) == 0) reinterpret_cast<uint8_t *>(a.rootmask)[gi >> 3] = (uint8_t)(nib | (hi << 4));
     }
 }
 
