@@ -98,11 +98,15 @@ __device__ __noinline__ bool bond_exact(float ti, float tj, double phi, double b
     return u < p;
 }
 
-// Filter: e = 2^(a * m2b) with m2b = -2 beta log2(e) in fp32 approximates 1 - p; v = 1 - u.
-// |e32 - e| < 4e-7 for a >= 0 at ANY beta (the relative error of the exponent is bounded through
-// x 2^-x <= 0.531, the ex2.approx error is 2^-22 relative), |v32 - v| < 3.1e-8.  With delta = 2e-6
-// the sign of (e32 - v32) settles the decision whenever |e32 - v32| > delta; otherwise (2 delta of
-// all bonds) fall back to the exact fp64 expression.
+// Filter (fp32): with sigma rounded to fp32, e32 = ex2.approx((sigma_i m2b) sigma_j), m2b = -2 beta
+// log2(e), approximates e = 1 - p = exp(-2 beta sigma_i sigma_j); f = 1 + v23 with v23 the top 23 bits
+// of 1 - u (taken from ~w), so d = (e32 + 1) - f approximates e - (1 - u) = p' ... and
+//     u < p  <=>  e < 1 - u  <=>  d < 0.
+// Error budget of d: the exponent x = a m2b carries a relative error < 4e-7 (three fp32 roundings
+// of sigma, two products, m2b itself), so |delta e| = e ln2 |x| 4e-7 <= 0.531 * 0.693 * 4e-7 = 1.5e-7
+// at ANY beta (x 2^-x <= 0.531); ex2.approx: 2^-22 relative, <= 2.4e-7; e32 + 1: 6e-8; truncation
+// of v to 23 bits: 1.2e-7; f subtracts exactly.  Total < 6e-7, so |d| > kFilterDelta = 2e-6 settles the
+// sign; otherwise (4e-6 of all bonds) the definition is evaluated in fp64 (bond_exact).
 constexpr float kFilterDelta = 2e-6f;
 
 struct BondCtx {
@@ -111,15 +115,13 @@ struct BondCtx {
     unsigned long long *fallback_counter;
 };
 
-__device__ __forceinline__ bool bond_decide(double a, uint32_t w, float ti, float tj, const BondCtx &cx)
+// gs = sigma_i * m2b (fp32), gj = sigma_j (fp32); returns d (see above)
+__device__ __forceinline__ float bond_filter(float gs, float gj, uint32_t w)
 {
-    const float af = __double2float_rn(a);
     float e;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(af * cx.m2b));
-    const float v = __uint2float_rn(~w) * 2.3283064365386963e-10f;   // (2^32-1-w) 2^-32 ~ 1-u
-    const float d = e - v;
-    if (fabsf(d) > kFilterDelta) return d < 0.0f;                    // e < 1-u  <=>  u < 1-e = p
-    return bond_exact(ti, tj, cx.phi, cx.beta, w, cx.fallback_counter);
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(gs * gj));
+    const float f = __uint_as_float(((~w) >> 9) | 0x3f800000u);
+    return (e + 1.0f) - f;
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -168,8 +168,8 @@ k_bonds(const SweepArgs a)
     static_assert(RS <= 32, "halo column is computed by one lane per row");
 
     __shared__ double2 tab[kTabN + 1];
-    __shared__ double h_c[NW][RS], h_s[NW][RS], h_g[NW][RS];
-    __shared__ float h_t[NW][RS];
+    __shared__ double h_c[NW][RS], h_s[NW][RS];
+    __shared__ float h_t[NW][RS], h_g[NW][RS];
     __shared__ double red[NW][6];
     __shared__ unsigned long long redc[NW][2];
     __shared__ bool is_last;
@@ -209,12 +209,12 @@ k_bonds(const SweepArgs a)
             h_t[warp][lane] = th;
             h_c[warp][lane] = c;
             h_s[warp][lane] = s;
-            h_g[warp][lane] = __fma_rn(c, cphi, s * sphi);
+            h_g[warp][lane] = __double2float_rn(__fma_rn(c, cphi, s * sphi));
         }
         __syncwarp();
 
-        float pt[VEC], nt[VEC];
-        double pc[VEC], ps[VEC], pg[VEC];
+        float pt[VEC], nt[VEC], pg[VEC];
+        double pc[VEC], ps[VEC];
         load_vec<VEC, true>(a.theta + (size_t)y0 * L + xl, pt);
         {
             uint32_t y1 = y0 + 1;
@@ -224,7 +224,7 @@ k_bonds(const SweepArgs a)
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
             sincos_tab(pt[v], tab, ps[v], pc[v]);
-            pg[v] = __fma_rn(pc[v], cphi, ps[v] * sphi);
+            pg[v] = __double2float_rn(__fma_rn(pc[v], cphi, ps[v] * sphi));
         }
 #pragma unroll 1
         for (int r = 1; r <= RS; ++r) {
@@ -237,16 +237,17 @@ k_bonds(const SweepArgs a)
                 if (y2 >= L) y2 -= L;
                 load_vec<VEC, true>(a.theta + (size_t)y2 * L + xl, nt);
             }
-            double c[VEC], s[VEC], g[VEC];
+            double c[VEC], s[VEC];
+            float g[VEC];
 #pragma unroll
             for (int v = 0; v < VEC; ++v) {
                 sincos_tab(ct[v], tab, s[v], c[v]);
-                g[v] = __fma_rn(c[v], cphi, s[v] * sphi);
+                g[v] = __double2float_rn(__fma_rn(c[v], cphi, s[v] * sphi));
             }
             const uint32_t gy = y0 + r - 1;                 // global row being finished
             double cn = __shfl_down_sync(0xffffffffu, pc[0], 1);
             double sn = __shfl_down_sync(0xffffffffu, ps[0], 1);
-            double gn = __shfl_down_sync(0xffffffffu, pg[0], 1);
+            float gn = __shfl_down_sync(0xffffffffu, pg[0], 1);
             float tn = __shfl_down_sync(0xffffffffu, pt[0], 1);
             if (lane == 31) { cn = h_c[warp][r - 1]; sn = h_s[warp][r - 1]; gn = h_g[warp][r - 1]; tn = h_t[warp][r - 1]; }
             uint32_t wx[VEC], wy[VEC];
@@ -259,12 +260,11 @@ k_bonds(const SweepArgs a)
                 }
             }
             uint32_t xn = 0, yn = 0;
+            float dx[VEC], dy[VEC], dmin = 1.0f;
 #pragma unroll
             for (int v = 0; v < VEC; ++v) {
                 const double c2 = (v + 1 < VEC) ? pc[(v + 1) % VEC] : cn;
                 const double s2 = (v + 1 < VEC) ? ps[(v + 1) % VEC] : sn;
-                const double g2 = (v + 1 < VEC) ? pg[(v + 1) % VEC] : gn;
-                const float t2 = (v + 1 < VEC) ? pt[(v + 1) % VEC] : tn;
                 aMx += pc[v];
                 aMy += ps[v];
                 aCx = __fma_rn(pc[v], c2, aCx);
@@ -276,8 +276,29 @@ k_bonds(const SweepArgs a)
                 aSy = __fma_rn(ps[v], c[v], aSy);
                 aSy = __fma_rn(-pc[v], s[v], aSy);
                 if constexpr (kBonds) {
-                    if (bond_decide(pg[v] * g2, wx[v], pt[v], t2, bcx)) xn |= 1u << v;
-                    if (bond_decide(pg[v] * g[v], wy[v], pt[v], ct[v], bcx)) yn |= 1u << v;
+                    const float g2 = (v + 1 < VEC) ? pg[(v + 1) % VEC] : gn;
+                    const float gs = pg[v] * bcx.m2b;
+                    dx[v] = bond_filter(gs, g2, wx[v]);
+                    dy[v] = bond_filter(gs, g[v], wy[v]);
+                    dmin = fminf(dmin, fminf(fabsf(dx[v]), fabsf(dy[v])));
+                    if (dx[v] < 0.0f) xn |= 1u << v;
+                    if (dy[v] < 0.0f) yn |= 1u << v;
+                }
+            }
+            if constexpr (kBonds) {
+                if (dmin <= kFilterDelta) {              // rare: some decision of this lane is too close to call in fp32
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) {
+                        const float t2 = (v + 1 < VEC) ? pt[(v + 1) % VEC] : tn;
+                        if (fabsf(dx[v]) <= kFilterDelta) {
+                            xn &= ~(1u << v);
+                            if (bond_exact(pt[v], t2, bcx.phi, bcx.beta, wx[v], bcx.fallback_counter)) xn |= 1u << v;
+                        }
+                        if (fabsf(dy[v]) <= kFilterDelta) {
+                            yn &= ~(1u << v);
+                            if (bond_exact(pt[v], ct[v], bcx.phi, bcx.beta, wy[v], bcx.fallback_counter)) yn |= 1u << v;
+                        }
+                    }
                 }
             }
             if constexpr (kBonds) {
