@@ -278,6 +278,10 @@ SweepArgs base_args(const xy_state *s)
     }
     a.seed_lo = (uint32_t)(s->seed & 0xffffffffu);
     a.seed_hi = (uint32_t)(s->seed >> 32);
+    for (uint32_t r = 0; r < 10; ++r) {
+        a.rk[2 * r] = a.seed_lo + r * 0x9E3779B9u;
+        a.rk[2 * r + 1] = a.seed_hi + r * 0xBB67AE85u;
+    }
     a.t = (uint32_t)s->T;
     a.sincos_tab = s->tab();
     return a;

@@ -37,6 +37,24 @@ __host__ __device__ __forceinline__ U4 philox4x32_10(uint32_t c0, uint32_t c1, u
     return U4{c0, c1, c2, c3};
 }
 
+// The same with the ten round keys precomputed (rk[2r] = k0 + r * 0x9E3779B9, rk[2r+1] = k1 + r * 0xBB67AE85):
+// as kernel arguments they are constant-bank operands of the XORs.
+__device__ __forceinline__ U4 philox4x32_10_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const uint32_t (&rk)[20])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk[2 * r];
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk[2 * r + 1];
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    return U4{c0, c1, c2, c3};
+}
+
 // counter = (idx lo, idx hi, (u32)t, tag); key = (seed lo, seed hi)
 __host__ __device__ __forceinline__ U4 rng(uint32_t seed_lo, uint32_t seed_hi, uint64_t idx, uint32_t t, uint32_t tag)
 {
@@ -96,6 +114,17 @@ __device__ __noinline__ bool bond_exact(float ti, float tj, double phi, double b
     const double u = __dmul_rn(__dadd_rn((double)w, 0.5), 1.0 / 4294967296.0);
     atomicAdd(fallback_counter, 1ULL);
     return u < p;
+}
+
+// The same for the bond of site (y, x) in direction dir (0: +x, 1: +y), angles re-read from memory
+// (the streaming loop does not keep them once (cos, sin, sigma) are evaluated).
+__device__ __noinline__ bool bond_exact_at(const float *theta, uint32_t L, uint32_t y, uint32_t x, int dir,
+                                           double phi, double beta, uint32_t w, unsigned long long *fallback_counter)
+{
+    uint32_t x2 = x, y2 = y;
+    if (dir == 0) { x2 = x + 1; if (x2 == L) x2 = 0; }
+    else { y2 = y + 1; if (y2 == L) y2 = 0; }
+    return bond_exact(theta[(size_t)y * L + x], theta[(size_t)y2 * L + x2], phi, beta, w, fallback_counter);
 }
 
 // Filter (fp32): with sigma rounded to fp32, e32 = ex2.approx((sigma_i m2b) sigma_j), m2b = -2 beta

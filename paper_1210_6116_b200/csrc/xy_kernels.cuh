@@ -58,6 +58,7 @@ struct SweepArgs {
     uint32_t     tiles_x, ntiles;
     uint32_t     Ldiv_mul, Ldiv_shift;   // d / L for d < 2^22: umulhi(d, Ldiv_mul) >> Ldiv_shift
     uint32_t     seed_lo, seed_hi;
+    uint32_t     rk[20];          // Philox round keys (k0, k1) of rounds 0..9, derived from the seed on the host
     uint32_t     t;               // sweep counter of THIS sweep (state before it has T = t sweeps done)
     int          beta_from_ctl;   // 1: read beta from ctl->beta (PCC), 0: use beta
     int          feed_pcc;        // 1: finalize feeds the observables of the incoming state to the controller
@@ -139,21 +140,21 @@ __device__ inline void pcc_feed(DevCtl *c, double N, double Cx, double Sx, doubl
 // computed once per strip by lanes 0..RS-1 into a per-warp shared slot.  Row RS of the strip (the
 // first row of the strip below) is recomputed as the y-halo (1/RS overhead).
 // ---------------------------------------------------------------------------------------------
-constexpr int kTabN = 256;                 // sincos table: entries k = 0..256 at angle 2 pi k / 256
+constexpr int kTabN = 1024;                // sincos table: entries k = 0..1024 at angle 2 pi k / 1024
 
-// sin, cos of an fp32 angle in [0, 2pi(1+1e-7)]: table lookup + degree-5/4 Taylor rotation in
-// fp64, |error| < 1e-15 (|x| <= pi/256: x^7/5040 = 8e-18, x^6/720 = 5e-15).
+// sin, cos of an fp32 angle in [0, 2pi(1+1e-7)]: table lookup + short Taylor rotation in fp64.
+// |x| <= pi/1024: sin x = x - x^3/6 (+2.3e-15), cos x - 1 = -x^2/2 + x^4/24 (+1.2e-18); the reduction
+// uses fl64(2 pi) k/1024 (exact scaling) for the table angle 2 pi k/1024: off by <= 2.5e-16.  |error| < 4e-15.
 __device__ __forceinline__ void sincos_tab(float theta, const double2 *tab, double &s, double &c)
 {
     const double t = (double)theta;
-    const double kd = __fma_rn(t, 40.743665431525208, 6755399441055744.0);      // 256/(2 pi), round to integer
+    const double kd = __fma_rn(t, 162.97466172610083, 6755399441055744.0);      // 1024/(2 pi), round to integer
     const int k = __double2loint(kd);
     const double kf = kd - 6755399441055744.0;
-    double x = __fma_rn(-kf, 0.02454369260617026, t);                          // fl64(2 pi)/256, exact scaling
-    x = __fma_rn(-kf, 9.5675529620887e-19, x);                                  // (2 pi - fl64(2 pi))/256
+    const double x = __fma_rn(-kf, 0.006135923151542565, t);                    // fl64(2 pi)/1024
     const double2 cs = tab[k];
     const double x2 = x * x;
-    const double sx = __fma_rn(x * x2, __fma_rn(x2, 8.3333333333333333e-3, -1.6666666666666667e-1), x);
+    const double sx = __fma_rn(x * x2, -1.6666666666666667e-1, x);
     const double dc = x2 * __fma_rn(x2, 4.1666666666666667e-2, -0.5);           // cos x - 1
     c = __fma_rn(-cs.y, sx, __fma_rn(cs.x, dc, cs.x));
     s = __fma_rn(cs.x, sx, __fma_rn(cs.y, dc, cs.y));
@@ -213,32 +214,29 @@ k_bonds(const SweepArgs a)
         }
         __syncwarp();
 
-        float pt[VEC], nt[VEC], pg[VEC];
-        double pc[VEC], ps[VEC];
-        load_vec<VEC, true>(a.theta + (size_t)y0 * L + xl, pt);
+        // two register sets (A, B) alternate as "row being finished" and "row below": no copies
+        float tA[VEC], tB[VEC], gA[VEC], gB[VEC];
+        double cA[VEC], sA[VEC], cB[VEC], sB[VEC];
+        load_vec<VEC, true>(a.theta + (size_t)y0 * L + xl, tA);
         {
             uint32_t y1 = y0 + 1;
             if (y1 >= L) y1 -= L;
-            load_vec<VEC, true>(a.theta + (size_t)y1 * L + xl, nt);
+            load_vec<VEC, true>(a.theta + (size_t)y1 * L + xl, tB);
         }
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
-            sincos_tab(pt[v], tab, ps[v], pc[v]);
-            pg[v] = __double2float_rn(__fma_rn(pc[v], cphi, ps[v] * sphi));
+            sincos_tab(tA[v], tab, sA[v], cA[v]);
+            gA[v] = __double2float_rn(__fma_rn(cA[v], cphi, sA[v] * sphi));
         }
-#pragma unroll 1
-        for (int r = 1; r <= RS; ++r) {
-            // this iteration finishes row r-1 (held in p*): its x bonds, and its y bonds with row r
-            float ct[VEC];
-#pragma unroll
-            for (int v = 0; v < VEC; ++v) ct[v] = nt[v];
+        // finishes row r-1 (evaluated, in pc/ps/pg): its x bonds, and its y bonds with row r, whose
+        // raw angles are in ct and whose (cos, sin, sigma) land in c/s/g; pt is free for the prefetch
+        auto step = [&](int r, float (&pt)[VEC], const double (&pc)[VEC], const double (&ps)[VEC], const float (&pg)[VEC],
+                        const float (&ct)[VEC], double (&c)[VEC], double (&s)[VEC], float (&g)[VEC]) {
             if (r < RS) {                                   // prefetch row r+1
                 uint32_t y2 = y0 + r + 1;
                 if (y2 >= L) y2 -= L;
-                load_vec<VEC, true>(a.theta + (size_t)y2 * L + xl, nt);
+                load_vec<VEC, true>(a.theta + (size_t)y2 * L + xl, pt);
             }
-            double c[VEC], s[VEC];
-            float g[VEC];
 #pragma unroll
             for (int v = 0; v < VEC; ++v) {
                 sincos_tab(ct[v], tab, s[v], c[v]);
@@ -248,21 +246,20 @@ k_bonds(const SweepArgs a)
             double cn = __shfl_down_sync(0xffffffffu, pc[0], 1);
             double sn = __shfl_down_sync(0xffffffffu, ps[0], 1);
             float gn = __shfl_down_sync(0xffffffffu, pg[0], 1);
-            float tn = __shfl_down_sync(0xffffffffu, pt[0], 1);
-            if (lane == 31) { cn = h_c[warp][r - 1]; sn = h_s[warp][r - 1]; gn = h_g[warp][r - 1]; tn = h_t[warp][r - 1]; }
+            if (lane == 31) { cn = h_c[warp][r - 1]; sn = h_s[warp][r - 1]; gn = h_g[warp][r - 1]; }
             uint32_t wx[VEC], wy[VEC];
             if constexpr (kBonds) {
 #pragma unroll
                 for (int v = 0; v < VEC; v += 2) {
                     const uint64_t site = (uint64_t)gy * L + xl + v;
-                    const U4 w = rng(a.seed_lo, a.seed_hi, site >> 1, a.t, TAG_BOND);
+                    const U4 w = philox4x32_10_rk((uint32_t)(site >> 1), (uint32_t)(site >> 33), a.t, TAG_BOND, a.rk);
                     wx[v] = w.x; wy[v] = w.y; wx[v + 1] = w.z; wy[v + 1] = w.w;
                 }
             }
             uint32_t xn = 0, yn = 0;
             float dx[VEC], dy[VEC], dmin = 1.0f;
 #pragma unroll
-            for (int v = 0; v < VEC; ++v) {
+            for (int v = VEC - 1; v >= 0; --v) {
                 const double c2 = (v + 1 < VEC) ? pc[(v + 1) % VEC] : cn;
                 const double s2 = (v + 1 < VEC) ? ps[(v + 1) % VEC] : sn;
                 aMx += pc[v];
@@ -281,27 +278,24 @@ k_bonds(const SweepArgs a)
                     dx[v] = bond_filter(gs, g2, wx[v]);
                     dy[v] = bond_filter(gs, g[v], wy[v]);
                     dmin = fminf(dmin, fminf(fabsf(dx[v]), fabsf(dy[v])));
-                    if (dx[v] < 0.0f) xn |= 1u << v;
-                    if (dy[v] < 0.0f) yn |= 1u << v;
+                    xn = __funnelshift_l(__float_as_uint(dx[v]), xn, 1);      // (xn << 1) | sign(dx): active iff d < 0
+                    yn = __funnelshift_l(__float_as_uint(dy[v]), yn, 1);
                 }
             }
             if constexpr (kBonds) {
                 if (dmin <= kFilterDelta) {              // rare: some decision of this lane is too close to call in fp32
 #pragma unroll
                     for (int v = 0; v < VEC; ++v) {
-                        const float t2 = (v + 1 < VEC) ? pt[(v + 1) % VEC] : tn;
                         if (fabsf(dx[v]) <= kFilterDelta) {
                             xn &= ~(1u << v);
-                            if (bond_exact(pt[v], t2, bcx.phi, bcx.beta, wx[v], bcx.fallback_counter)) xn |= 1u << v;
+                            if (bond_exact_at(a.theta, L, gy, xl + v, 0, bcx.phi, bcx.beta, wx[v], bcx.fallback_counter)) xn |= 1u << v;
                         }
                         if (fabsf(dy[v]) <= kFilterDelta) {
                             yn &= ~(1u << v);
-                            if (bond_exact(pt[v], ct[v], bcx.phi, bcx.beta, wy[v], bcx.fallback_counter)) yn |= 1u << v;
+                            if (bond_exact_at(a.theta, L, gy, xl + v, 1, bcx.phi, bcx.beta, wy[v], bcx.fallback_counter)) yn |= 1u << v;
                         }
                     }
                 }
-            }
-            if constexpr (kBonds) {
                 nbx += __popc(xn);
                 nby += __popc(yn);
                 if constexpr (VEC == 4) {
@@ -313,8 +307,12 @@ k_bonds(const SweepArgs a)
                     if ((lane & 1) == 0) a.bonds[((size_t)gy * L + xl) >> 2] = (uint8_t)(mine | (other << 2));
                 }
             }
-#pragma unroll
-            for (int v = 0; v < VEC; ++v) { pc[v] = c[v]; ps[v] = s[v]; pg[v] = g[v]; pt[v] = ct[v]; }
+        };
+        static_assert(RS % 2 == 0, "the row loop is unrolled by two");
+#pragma unroll 1
+        for (int r = 1; r <= RS; r += 2) {
+            step(r, tA, cA, sA, gA, tB, cB, sB, gB);
+            step(r + 1, tB, cB, sB, gB, tA, cA, sA, gA);
         }
     }
 
