@@ -541,9 +541,9 @@ k_label(const SweepArgs a)
             const int rt = (1 << (j - 1)) - 1 + (kb << j);     // upper row of the boundary
             const int col0 = it * cpi, ww = col0 >> 5, off = col0 & 31;
             uint32_t need = Ns[rt][ww] & (((1u << cpi) - 1u) << off);
+            const uint32_t bt = rt * TW + 32 * ww;
             if (need) {
                 const uint32_t St = Ss[rt][ww], Sb = Ss[rt + 1][ww];
-                const uint32_t bt = rt * TW + 32 * ww;
                 do {
                     const int c = __ffs(need) - 1;
                     need &= need - 1;
@@ -558,22 +558,19 @@ k_label(const SweepArgs a)
         __syncthreads();
     }
 
-    // ---- flatten by pointer jumping over ALL entries (fixed cost, no divergence): parent[i] <-
-    //      parent[parent[i]] until nothing changes.  In place: a racing reader sees an ancestor.
-    for (;;) {
-        bool changed = false;
+    // ---- flatten: ONE pass of parent[i] <- parent[parent[i]] over all entries (fixed cost, no
+    //      divergence; the wave order leaves most chains at length <= 2), emit walks what is left.
+    //      In place: a racing reader sees an ancestor.
+    {
 #pragma unroll 2
         for (int k = 0; k < TH / RPP; ++k) {
             const uint32_t i0 = (k * RPP + rq) * TW + 4 * q;
             const uint4 p1 = *reinterpret_cast<const uint4 *>(&parent[i0]);
             uint4 p2;
             p2.x = parent[p1.x]; p2.y = parent[p1.y]; p2.z = parent[p1.z]; p2.w = parent[p1.w];
-            if (p2.x != p1.x || p2.y != p1.y || p2.z != p1.z || p2.w != p1.w) {
-                *reinterpret_cast<uint4 *>(&parent[i0]) = p2;
-                changed = true;
-            }
+            *reinterpret_cast<uint4 *>(&parent[i0]) = p2;
         }
-        if (!__syncthreads_or(changed)) break;
+        __syncthreads();
     }
 
     // ---- emit: label = global index of the root; rootmask bit = "I am the tile-local root" ----
@@ -583,7 +580,16 @@ k_label(const SweepArgs a)
         const int row = k * RPP + rq;
         const uint32_t i0 = row * TW + 4 * q;
         const uint4 rt = *reinterpret_cast<const uint4 *>(&parent[i0]);
-        const uint32_t root[4] = {rt.x, rt.y, rt.z, rt.w};
+        uint32_t root[4] = {rt.x, rt.y, rt.z, rt.w};
+        {
+            uint32_t up[4];
+#pragma unroll
+            for (int v = 0; v < 4; ++v) up[v] = parent[root[v]];
+            while (up[0] != root[0] || up[1] != root[1] || up[2] != root[2] || up[3] != root[3]) {   // rare: a longer chain
+#pragma unroll
+                for (int v = 0; v < 4; ++v) { root[v] = up[v]; up[v] = parent[root[v]]; }
+            }
+        }
         LabelT out[4];
         uint32_t nib = 0;
 #pragma unroll
@@ -650,7 +656,10 @@ k_merge(const SweepArgs a)
 //           and rows in which nothing flipped are not written back.
 // ---------------------------------------------------------------------------------------------
 template <int WPR, int TH, typename LabelT>
-__global__ void __launch_bounds__(WPR * TH, (sizeof(LabelT) == 4 ? 768 : 512) / (WPR * TH))
+#ifndef XY_EXP_FLIPT
+#define XY_EXP_FLIPT 1024
+#endif
+__global__ void __launch_bounds__(WPR * TH, (sizeof(LabelT) == 4 ? XY_EXP_FLIPT : 512) / (WPR * TH))
 k_flip(const SweepArgs a)
 {
     constexpr int TW = 32 * WPR, NT = WPR * TH;
