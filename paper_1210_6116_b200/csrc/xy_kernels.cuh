@@ -656,10 +656,7 @@ k_merge(const SweepArgs a)
 //           and rows in which nothing flipped are not written back.
 // ---------------------------------------------------------------------------------------------
 template <int WPR, int TH, typename LabelT>
-#ifndef XY_EXP_FLIPT
-#define XY_EXP_FLIPT 1024
-#endif
-__global__ void __launch_bounds__(WPR * TH, (sizeof(LabelT) == 4 ? XY_EXP_FLIPT : 512) / (WPR * TH))
+__global__ void __launch_bounds__(WPR * TH, (sizeof(LabelT) == 4 ? 1536 : 1024) / (WPR * TH))
 k_flip(const SweepArgs a)
 {
     constexpr int TW = 32 * WPR, NT = WPR * TH;
@@ -691,32 +688,32 @@ k_flip(const SweepArgs a)
         }
     }
 
-    LabelT lab[NP][4];
-    uint32_t rb = 0;                                 // root bits of my 4 sites in pass k: nibble k
-#pragma unroll
-    for (int k = 0; k < NP; ++k) {
-        const int row = k * RPP + rq;
-        const size_t i = (size_t)(y0 + row) * L + x0 + 4 * q;
+    // labels are read twice (here and in the last phase; the second read hits L1/L2) rather than
+    // held in registers: few registers, so many CTAs per SM hide the latency of the phases
+    auto load_labels = [&](size_t i, LabelT (&lab)[4]) {
         if constexpr (sizeof(LabelT) == 4) {
             const uint4 v = __ldg(reinterpret_cast<const uint4 *>(labels + i));
-            lab[k][0] = v.x; lab[k][1] = v.y; lab[k][2] = v.z; lab[k][3] = v.w;
+            lab[0] = v.x; lab[1] = v.y; lab[2] = v.z; lab[3] = v.w;
         } else {
             const ulonglong2 u = __ldg(reinterpret_cast<const ulonglong2 *>(labels + i));
             const ulonglong2 v = __ldg(reinterpret_cast<const ulonglong2 *>(labels + i + 2));
-            lab[k][0] = u.x; lab[k][1] = u.y; lab[k][2] = v.x; lab[k][3] = v.y;
+            lab[0] = u.x; lab[1] = u.y; lab[2] = v.x; lab[3] = v.y;
         }
-        const uint32_t nib = (__ldg(reinterpret_cast<const uint8_t *>(a.rootmask) + (i >> 3)) >> (i & 4u)) & 15u;
-        rb |= nib << (4 * k);
-    }
-
+    };
+    uint32_t rb = 0;                                 // root bits of my 4 sites in pass k: nibble k
     // ---- tile roots that k_merge linked elsewhere are queued; the others are the clusters ----
     uint32_t merged = 0;
 #pragma unroll
     for (int k = 0; k < NP; ++k) {
-        const LabelT own = gbase + (LabelT)(k * RPP + rq) * L + 4 * q;
+        const int row = k * RPP + rq;
+        const size_t i = (size_t)(y0 + row) * L + x0 + 4 * q;
+        LabelT lab[4];
+        load_labels(i, lab);
+        const uint32_t nib = (__ldg(reinterpret_cast<const uint8_t *>(a.rootmask) + (i >> 3)) >> (i & 4u)) & 15u;
+        rb |= nib << (4 * k);
 #pragma unroll
         for (int v = 0; v < 4; ++v)
-            if (lab[k][v] != own + v) merged |= 1u << (4 * k + v);
+            if (lab[v] != (LabelT)(i + v)) merged |= 1u << (4 * k + v);
     }
     merged &= rb;
     const uint32_t ncl = __popc(rb & ~merged);
@@ -753,13 +750,15 @@ k_flip(const SweepArgs a)
         const size_t i = (size_t)(y0 + row) * L + x0 + 4 * q;
         const float4 t4 = *reinterpret_cast<const float4 *>(a.theta + i);
         const float th[4] = {t4.x, t4.y, t4.z, t4.w};
+        LabelT lab[4];
+        load_labels(i, lab);
         float out[4];
         bool any = false;
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
             uint32_t loc = loc0 + v;
             if (!((rb >> (4 * k + v)) & 1u)) {
-                const uint32_t d = (uint32_t)(lab[k][v] - gbase);          // r*L + c, < TH*L <= 2^22
+                const uint32_t d = (uint32_t)(lab[v] - gbase);          // r*L + c, < TH*L <= 2^22
                 const uint32_t rr = __umulhi(d, a.Ldiv_mul) >> a.Ldiv_shift;
                 loc = d - rr * Lm;
             }
