@@ -50,9 +50,9 @@ def bytes_model(L, label_bytes, tw, th):
     w = label_bytes
     return {
         "k_bonds": 4.0 + 0.25,                                  # theta read, packed bond bits written
-        "k_label": 0.25 + w,                                    # bond bits read, provisional label written
+        "k_label": 0.25 + w + 0.125,                            # bond bits read, provisional label + root bit written
         "k_merge": (tw + th) * (2.0 * w + 0.125) / (tw * th),   # two labels + the bond bit per tile-edge site
-        "k_flip": w + 4.0 + 4.0,                                # label read, theta read, theta written
+        "k_flip": w + 0.125 + 4.0 + 4.0,                        # label + root bit read, theta read, theta written
     }
 
 
