@@ -165,6 +165,49 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+class RankGroup:
+    """The multi-process plumbing of --gpus N: N independent replicas (seed + rank), one process per
+    GPU, no data-path collective.  The process group serves only the barrier around the timed region
+    and the max-over-ranks of the device time.  backend "nccl" on the GPUs; "gloo" with device "cpu"
+    in the CPU tests (tests/test_bench_ranks_cpu.py)."""
+
+    def __init__(self, rank, world, backend="nccl", device=None, sync=None):
+        self.rank, self.world, self.device, self.sync = rank, world, device, sync
+        self.dist = None
+        if world > 1:
+            import torch
+            import torch.distributed as dist
+            kw = {"device_id": device} if backend == "nccl" else {}
+            dist.init_process_group(backend, rank=rank, world_size=world, **kw)
+            self.dist, self.torch = dist, torch
+
+    def barrier(self):
+        if self.dist is not None:
+            self.dist.barrier()
+        if self.sync is not None:
+            self.sync()
+
+    def max_over_ranks(self, x):
+        if self.dist is None:
+            return x
+        t = self.torch.tensor([x], dtype=self.torch.float64, device=self.device)
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def close(self):
+        if self.dist is not None:
+            self.dist.destroy_process_group()
+
+
+def replica_seed(seed, rank):
+    return seed + rank
+
+
+def whole_job_value(world, N, K, ms):
+    """spin updates/s of the whole job: every replica did K sweeps of N sites in (max over ranks) ms."""
+    return world * N * K / (ms * 1e-3)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -187,26 +230,13 @@ def main():
         return
 
     import torch
-    import torch.distributed as dist
     import paper_1210_6116_b200 as xy
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (the product path has no CPU fallback)")
     torch.cuda.set_device(local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    grp = RankGroup(rank, world, "nccl", torch.device("cuda", local_rank), torch.cuda.synchronize)
+    barrier, max_over_ranks = grp.barrier, grp.max_over_ranks
 
     cfg_idx, L, init, seed, beta, therm = WORKLOADS[args.workload]
     N = L * L
@@ -215,7 +245,7 @@ def main():
     tw, th = (128, 64) if L % 128 == 0 else (64, 64)
     K, W = args.steps, max(args.warmup, 0)
 
-    st = xy.XYState(L, seed + rank, xy_inputs.INIT_CODE[init], flags=flags)
+    st = xy.XYState(L, replica_seed(seed, rank), xy_inputs.INIT_CODE[init], flags=flags)
     if therm:
         st.sw_sweeps(beta, therm)
     st.sw_sweeps(beta, W)
@@ -234,7 +264,7 @@ def main():
     ms = max_over_ranks(e0.elapsed_time(e1))
     launches = st.get_launch_count() - launches0
     clocks = sampler.stop()
-    value = world * N * K / (ms * 1e-3)
+    value = whole_job_value(world, N, K, ms)
     obs = st.measure()
 
     # ---- timed region 2: the same K sweeps with CUDA events around every kernel ----
@@ -319,8 +349,7 @@ def main():
         }
         print(json.dumps(line), flush=True)
     st.destroy()
-    if world > 1:
-        dist.destroy_process_group()
+    grp.close()
 
 
 if __name__ == "__main__":
