@@ -55,7 +55,7 @@
 #define XYO_TWO_PI 6.283185307179586  /* 0x401921FB54442D18, fl64(2 pi) */
 #define XYO_PI     3.141592653589793  /* 0x400921FB54442D18, fl64(pi)   */
 
-enum { XYO_TAG_INIT = 0, XYO_TAG_DIR = 1, XYO_TAG_BOND = 2, XYO_TAG_FLIP = 3 };
+enum { XYO_TAG_INIT = 0, XYO_TAG_DIR = 1, XYO_TAG_BOND = 2, XYO_TAG_FLIP = 3, XYO_TAG_BOND_LO = 4 };
 
 /* ------------------------------------------------------------------------- */
 /* O1. RNG: Philox4x32 with 10 rounds (Salmon, Moraes, Dror, Shaw, SC'11).     */
@@ -147,14 +147,19 @@ double xyo_bond_prob(double beta, double sigma_i, double sigma_j)
     return -expm1(x);
 }
 
-/* uniforms of site i at sweep t: one Philox call per PAIR of sites q = i>>1;
- * even site takes words 0 (x bond) and 1 (y bond), odd site words 2 and 3.   */
+/* uniforms of site i at sweep t.  Two Philox calls per QUAD of sites q = i>>2, */
+/* A = rng(seed, q, t, BOND) and B = rng(seed, q, t, BOND_LO); site 4q+j takes   */
+/* the 32-bit words  wx = (lo16(A_j) << 16) | lo16(B_j)  (x bond) and            */
+/* wy = (hi16(A_j) << 16) | hi16(B_j)  (y bond):  call A holds the 16 leading    */
+/* bits of all 8 uniforms of the quad, call B the 16 trailing bits.              */
 void xyo_bond_uniforms_site(uint64_t seed, uint64_t t, uint64_t i, double *ux, double *uy)
 {
-    uint32_t w[4];
-    xyo_rng(seed, i >> 1, t, XYO_TAG_BOND, w);
-    if ((i & 1u) == 0) { *ux = xyo_uniform(w[0]); *uy = xyo_uniform(w[1]); }
-    else               { *ux = xyo_uniform(w[2]); *uy = xyo_uniform(w[3]); }
+    uint32_t A[4], B[4];
+    unsigned j = (unsigned)(i & 3u);
+    xyo_rng(seed, i >> 2, t, XYO_TAG_BOND, A);
+    xyo_rng(seed, i >> 2, t, XYO_TAG_BOND_LO, B);
+    *ux = xyo_uniform(((A[j] & 0xffffu) << 16) | (B[j] & 0xffffu));
+    *uy = xyo_uniform((A[j] & 0xffff0000u) | (B[j] >> 16));
 }
 
 static uint64_t right_of(uint64_t x, uint64_t y, uint64_t L) { return y * L + ((x + 1) % L); }

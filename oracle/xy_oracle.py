@@ -102,7 +102,7 @@ _run = _sig("xyo_run", C.c_int,
             [f32p, C.c_uint32, C.c_uint64, C.c_uint64, C.c_double, C.c_uint64,
              C.c_int, C.c_double, C.c_void_p])
 
-TAG_INIT, TAG_DIR, TAG_BOND, TAG_FLIP = 0, 1, 2, 3
+TAG_INIT, TAG_DIR, TAG_BOND, TAG_FLIP, TAG_BOND_LO = 0, 1, 2, 3, 4
 INIT_COLD, INIT_HOT = 0, 1
 
 

@@ -10,7 +10,7 @@ namespace xy {
 constexpr double kTwoPi = 6.283185307179586;   // fl64(2 pi)
 constexpr double kPi    = 3.141592653589793;   // fl64(pi)
 
-enum : uint32_t { TAG_INIT = 0, TAG_DIR = 1, TAG_BOND = 2, TAG_FLIP = 3 };
+enum : uint32_t { TAG_INIT = 0, TAG_DIR = 1, TAG_BOND = 2, TAG_FLIP = 3, TAG_BOND_LO = 4 };
 
 // ---------------------------------------------------------------------------------------------
 // Philox4x32 with 10 rounds (Salmon et al., SC'11).  Counter (c0..c3), key (k0,k1).
@@ -127,16 +127,18 @@ __device__ __noinline__ bool bond_exact_at(const float *theta, uint32_t L, uint3
     return bond_exact(theta[(size_t)y * L + x], theta[(size_t)y2 * L + x2], phi, beta, w, fallback_counter);
 }
 
-// Filter (fp32): with sigma rounded to fp32, e32 = ex2.approx((sigma_i m2b) sigma_j), m2b = -2 beta
-// log2(e), approximates e = 1 - p = exp(-2 beta sigma_i sigma_j); f = 1 + v23 with v23 the top 23 bits
-// of 1 - u (taken from ~w), so d = (e32 + 1) - f approximates e - (1 - u) = p' ... and
+// Filter (fp32, on the 16 leading bits of u): with sigma rounded to fp32, e32 = ex2.approx((sigma_i
+// m2b) sigma_j), m2b = -2 beta log2(e), approximates e = 1 - p = exp(-2 beta sigma_i sigma_j);
+// f = 1 + v with v = ((65535 - h) + 0.5) 2^-16 the midpoint of the interval that 1 - u lies in when only
+// the leading 16 bits h of the random word are known, so d = (e32 + 1) - f approximates e - (1 - u), and
 //     u < p  <=>  e < 1 - u  <=>  d < 0.
-// Error budget of d: the exponent x = a m2b carries a relative error < 4e-7 (three fp32 roundings
-// of sigma, two products, m2b itself), so |delta e| = e ln2 |x| 4e-7 <= 0.531 * 0.693 * 4e-7 = 1.5e-7
-// at ANY beta (x 2^-x <= 0.531); ex2.approx: 2^-22 relative, <= 2.4e-7; e32 + 1: 6e-8; truncation
-// of v to 23 bits: 1.2e-7; f subtracts exactly.  Total < 6e-7, so |d| > kFilterDelta = 2e-6 settles the
-// sign; otherwise (4e-6 of all bonds) the definition is evaluated in fp64 (bond_exact).
-constexpr float kFilterDelta = 2e-6f;
+// Error budget of d: the exponent x = a m2b carries a relative error < 4e-7 (three fp32 roundings of
+// sigma, two products, m2b itself), so |delta e| = e ln2 |x| 4e-7 <= 0.531 * 0.693 * 4e-7 = 1.5e-7 at
+// ANY beta (x 2^-x <= 0.531); ex2.approx: 2^-22 relative, <= 2.4e-7; e32 + 1: 6e-8; f subtracts
+// exactly; the unknown trailing bits of u: 2^-17 = 7.7e-6.  Total < 8.3e-6, so |d| > kFilterDelta = 1e-5
+// settles the sign; otherwise (2e-5 of all bonds) the trailing bits are drawn and the definition is
+// evaluated in fp64 (bond_exact).
+constexpr float kFilterDelta = 1e-5f;
 
 struct BondCtx {
     double phi, beta;
@@ -144,12 +146,13 @@ struct BondCtx {
     unsigned long long *fallback_counter;
 };
 
-// gs = sigma_i * m2b (fp32), gj = sigma_j (fp32); returns d (see above)
-__device__ __forceinline__ float bond_filter(float gs, float gj, uint32_t w)
+// gs = sigma_i * m2b (fp32), gj = sigma_j (fp32); hs holds the 16 leading bits h of the random word
+// at bit positions 7..22 (other bits arbitrary); returns d (see above)
+__device__ __forceinline__ float bond_filter(float gs, float gj, uint32_t hs)
 {
     float e;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(gs * gj));
-    const float f = __uint_as_float(((~w) >> 9) | 0x3f800000u);
+    const float f = __uint_as_float(((~hs) & 0x007fff80u) | 0x3f800040u);
     return (e + 1.0f) - f;
 }
 

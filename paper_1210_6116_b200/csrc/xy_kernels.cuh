@@ -247,14 +247,14 @@ k_bonds(const SweepArgs a)
             double sn = __shfl_down_sync(0xffffffffu, ps[0], 1);
             float gn = __shfl_down_sync(0xffffffffu, pg[0], 1);
             if (lane == 31) { cn = h_c[warp][r - 1]; sn = h_s[warp][r - 1]; gn = h_g[warp][r - 1]; }
-            uint32_t wx[VEC], wy[VEC];
+            // leading 16 bits of the 2 VEC uniforms: word j of call A of the quad serves site 4q+j
+            // (x: low half, y: high half); the trailing bits (call B) are drawn only on a close call
+            uint32_t wa[VEC];
+            const uint64_t site0 = (uint64_t)gy * L + xl;
             if constexpr (kBonds) {
-#pragma unroll
-                for (int v = 0; v < VEC; v += 2) {
-                    const uint64_t site = (uint64_t)gy * L + xl + v;
-                    const U4 w = philox4x32_10_rk((uint32_t)(site >> 1), (uint32_t)(site >> 33), a.t, TAG_BOND, a.rk);
-                    wx[v] = w.x; wy[v] = w.y; wx[v + 1] = w.z; wy[v + 1] = w.w;
-                }
+                const U4 w = philox4x32_10_rk((uint32_t)(site0 >> 2), (uint32_t)(site0 >> 34), a.t, TAG_BOND, a.rk);
+                if constexpr (VEC == 4) { wa[0] = w.x; wa[1] = w.y; wa[2] = w.z; wa[3] = w.w; }
+                else { const bool up = (site0 & 2u) != 0; wa[0] = up ? w.z : w.x; wa[1] = up ? w.w : w.y; }
             }
             uint32_t xn = 0, yn = 0;
             float dx[VEC], dy[VEC], dmin = 1.0f;
@@ -275,24 +275,30 @@ k_bonds(const SweepArgs a)
                 if constexpr (kBonds) {
                     const float g2 = (v + 1 < VEC) ? pg[(v + 1) % VEC] : gn;
                     const float gs = pg[v] * bcx.m2b;
-                    dx[v] = bond_filter(gs, g2, wx[v]);
-                    dy[v] = bond_filter(gs, g[v], wy[v]);
+                    dx[v] = bond_filter(gs, g2, wa[v] << 7);
+                    dy[v] = bond_filter(gs, g[v], wa[v] >> 9);
                     dmin = fminf(dmin, fminf(fabsf(dx[v]), fabsf(dy[v])));
                     xn = __funnelshift_l(__float_as_uint(dx[v]), xn, 1);      // (xn << 1) | sign(dx): active iff d < 0
                     yn = __funnelshift_l(__float_as_uint(dy[v]), yn, 1);
                 }
             }
             if constexpr (kBonds) {
-                if (dmin <= kFilterDelta) {              // rare: some decision of this lane is too close to call in fp32
+                if (dmin <= kFilterDelta) {              // rare: some decision of this lane is too close to call
+                    const U4 w = philox4x32_10_rk((uint32_t)(site0 >> 2), (uint32_t)(site0 >> 34), a.t, TAG_BOND_LO, a.rk);
+                    uint32_t wb[VEC];
+                    if constexpr (VEC == 4) { wb[0] = w.x; wb[1] = w.y; wb[2] = w.z; wb[3] = w.w; }
+                    else { const bool up = (site0 & 2u) != 0; wb[0] = up ? w.z : w.x; wb[1] = up ? w.w : w.y; }
 #pragma unroll
                     for (int v = 0; v < VEC; ++v) {
                         if (fabsf(dx[v]) <= kFilterDelta) {
+                            const uint32_t wx = (wa[v] << 16) | (wb[v] & 0xffffu);
                             xn &= ~(1u << v);
-                            if (bond_exact_at(a.theta, L, gy, xl + v, 0, bcx.phi, bcx.beta, wx[v], bcx.fallback_counter)) xn |= 1u << v;
+                            if (bond_exact_at(a.theta, L, gy, xl + v, 0, bcx.phi, bcx.beta, wx, bcx.fallback_counter)) xn |= 1u << v;
                         }
                         if (fabsf(dy[v]) <= kFilterDelta) {
+                            const uint32_t wy = (wa[v] & 0xffff0000u) | (wb[v] >> 16);
                             yn &= ~(1u << v);
-                            if (bond_exact_at(a.theta, L, gy, xl + v, 1, bcx.phi, bcx.beta, wy[v], bcx.fallback_counter)) yn |= 1u << v;
+                            if (bond_exact_at(a.theta, L, gy, xl + v, 1, bcx.phi, bcx.beta, wy, bcx.fallback_counter)) yn |= 1u << v;
                         }
                     }
                 }

@@ -89,13 +89,17 @@ def test_uniform_exact_and_open_interval():
 
 
 def test_bond_uniform_pairing():
-    """one Philox call per pair of sites; even site words 0,1, odd site words 2,3."""
+    """two Philox calls per quad of sites: call BOND holds the 16 leading bits of the quad's 8 uniforms,
+    call BOND_LO the 16 trailing bits; site 4q+j takes word j (x: low halves, y: high halves)."""
     seed, t = 99, 17
-    for i in (0, 1, 2, 3, 4094, 4095, (1 << 32) + 6, (1 << 32) + 7):
-        w = xo.rng(seed, i >> 1, t, xo.TAG_BOND)
+    for i in (0, 1, 2, 3, 4, 4093, 4094, 4095, (1 << 32) + 6, (1 << 32) + 7):
+        A = xo.rng(seed, i >> 2, t, xo.TAG_BOND)
+        B = xo.rng(seed, i >> 2, t, xo.TAG_BOND_LO)
         ux, uy = xo.bond_uniforms_site(seed, t, i)
-        a, b = (w[0], w[1]) if i % 2 == 0 else (w[2], w[3])
-        assert ux == (float(a) + 0.5) / 2 ** 32 and uy == (float(b) + 0.5) / 2 ** 32
+        j = i % 4
+        wx = ((int(A[j]) & 0xffff) << 16) | (int(B[j]) & 0xffff)
+        wy = (int(A[j]) & 0xffff0000) | (int(B[j]) >> 16)
+        assert ux == (float(wx) + 0.5) / 2 ** 32 and uy == (float(wy) + 0.5) / 2 ** 32
 
 
 def test_uniform_moments():
@@ -108,6 +112,25 @@ def test_uniform_moments():
     h, _ = np.histogram(u, bins=64, range=(0, 1))
     chi2 = ((h - n / 64) ** 2 / (n / 64)).sum()
     assert chi2 < 63 + 5 * np.sqrt(2 * 63)
+
+
+def test_bond_uniforms_uncorrelated_within_quad():
+    """the 8 uniforms of a quad come from two calls (leading / trailing halves): no correlation between
+    the x and y uniform of a site, between neighbouring sites of a quad, or between quads."""
+    seed, n = 5, 1 << 16
+    u = np.array([xo.bond_uniforms_site(seed, 3, i) for i in range(n)]) - 0.5     # [n, 2]
+    lim = 5.0 / 12.0 / np.sqrt(n)
+    assert abs((u[:, 0] * u[:, 1]).mean()) < lim                                    # x vs y of a site
+    for lag in (1, 2, 3, 4):
+        assert abs((u[:-lag, 0] * u[lag:, 0]).mean()) < lim
+        assert abs((u[:-lag, 1] * u[lag:, 1]).mean()) < lim
+        assert abs((u[:-lag, 0] * u[lag:, 1]).mean()) < lim
+    # leading and trailing halves of one uniform are independent: 16 x 16 coarse contingency
+    w = np.floor((u[:, 0] + 0.5) * 2 ** 32).astype(np.uint64)
+    hi, lo = (w >> 28) & 15, (w >> 12) & 15
+    h = np.zeros((16, 16)); np.add.at(h, (hi.astype(int), lo.astype(int)), 1)
+    chi2 = ((h - n / 256) ** 2 / (n / 256)).sum()
+    assert chi2 < 255 + 5 * np.sqrt(2 * 255)
 
 
 def test_hot_init():
