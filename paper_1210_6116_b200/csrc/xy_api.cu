@@ -124,7 +124,10 @@ struct KS {
     }
 };
 
-constexpr int kR = 8, kNW = 8;   // label / flip tiles: 8 warps x 8 rows = 128 x 64 (VEC 4) or 64 x 64 (VEC 2)
+#ifndef XY_EXP_KR
+#define XY_EXP_KR 8
+#endif
+constexpr int kR = XY_EXP_KR, kNW = 8;   // label / flip tiles: 8 warps x 8 rows = 128 x 64 (VEC 4) or 64 x 64 (VEC 2)
 
 Kernels pick_kernels(uint32_t L, bool l64)
 {

@@ -449,8 +449,13 @@ __device__ __forceinline__ void sunion_v(uint32_t *p, uint32_t a, uint32_t b)
 {
     volatile uint32_t *vp = p;
     for (;;) {
+#ifdef XY_EXP_NOHALVE
+        a = sfind_v(vp, a);
+        b = sfind_v(vp, b);
+#else
         a = sfind_h(vp, a);
         b = sfind_h(vp, b);
+#endif
         if (a == b) return;
         const uint32_t hi = a > b ? a : b, lo = a > b ? b : a;
         const uint32_t old = atomicMin(&p[hi], lo);
@@ -627,25 +632,37 @@ k_merge(const SweepArgs a)
     const uint32_t L = a.L;
     LabelT *labels = reinterpret_cast<LabelT *>(a.labels);
     const uint64_t total = (uint64_t)a.ntiles * (TW + TH);
-    for (uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; k < total; k += (uint64_t)gridDim.x * blockDim.x) {
-        const uint32_t tile = (uint32_t)(k / (TW + TH));
-        const uint32_t e = (uint32_t)(k - (uint64_t)tile * (TW + TH));
-        const uint32_t ty = tile / a.tiles_x, tx = tile - ty * a.tiles_x;
-        uint32_t x, y, x2, y2, bit;
-        if (e < TH) {
-            x = tx * TW + TW - 1; y = ty * TH + e;
-            x2 = x + 1 == L ? 0 : x + 1; y2 = y;
-            bit = 3;                                   // bx of the 4th site of its byte
-        } else {
-            x = tx * TW + (e - TH); y = ty * TH + TH - 1;
-            x2 = x; y2 = y + 1 == L ? 0 : y + 1;
-            bit = 4 + (x & 3u);
+    const uint64_t total_up = (total + 31u) & ~(uint64_t)31u;                  // whole warps stay in the loop (shuffles)
+    for (uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; k < total_up; k += (uint64_t)gridDim.x * blockDim.x) {
+        bool active = false;
+        LabelT la = 0, lb = 0;
+        if (k < total) {
+            const uint32_t tile = (uint32_t)(k / (TW + TH));
+            const uint32_t e = (uint32_t)(k - (uint64_t)tile * (TW + TH));
+            const uint32_t ty = tile / a.tiles_x, tx = tile - ty * a.tiles_x;
+            uint32_t x, y, x2, y2, bit;
+            if (e < TH) {
+                x = tx * TW + TW - 1; y = ty * TH + e;
+                x2 = x + 1 == L ? 0 : x + 1; y2 = y;
+                bit = 3;                                   // bx of the 4th site of its byte
+            } else {
+                x = tx * TW + (e - TH); y = ty * TH + TH - 1;
+                x2 = x; y2 = y + 1 == L ? 0 : y + 1;
+                bit = 4 + (x & 3u);
+            }
+            const size_t i = (size_t)y * L + x;
+            if ((a.bonds[i >> 2] >> bit) & 1u) {
+                active = true;
+                la = gload(labels + i);
+                lb = gload(labels + (size_t)y2 * L + x2);
+            }
         }
-        const size_t i = (size_t)y * L + x;
-        if ((a.bonds[i >> 2] >> bit) & 1u) {
-            const size_t j = (size_t)y2 * L + x2;
-            gunion<LabelT>(labels, gload(labels + i), gload(labels + j));
-        }
+        // neighbouring edge bonds mostly join the same two tile-local components: the lane to the
+        // left already does that union (it never skips unless ITS left neighbour does the same one)
+        const LabelT pa = __shfl_up_sync(0xffffffffu, la, 1), pb = __shfl_up_sync(0xffffffffu, lb, 1);
+        const bool pact = __shfl_up_sync(0xffffffffu, (int)active, 1) != 0;
+        const bool dup = (threadIdx.x & 31) != 0 && pact && pa == la && pb == lb;
+        if (active && !dup) gunion<LabelT>(labels, la, lb);
     }
 }
 
