@@ -242,7 +242,7 @@ def main():
     N = L * L
     flags = xy.FLAG_LABELS64 if args.labels64 else 0
     label_bytes = 8 if args.labels64 else 4
-    tw, th = (128, 64) if L % 128 == 0 else (64, 64)
+    tw, th = (128, 32) if L % 128 == 0 else (64, 32)
     K, W = args.steps, max(args.warmup, 0)
 
     st = xy.XYState(L, replica_seed(seed, rank), xy_inputs.INIT_CODE[init], flags=flags)

@@ -124,10 +124,7 @@ struct KS {
     }
 };
 
-#ifndef XY_EXP_KR
-#define XY_EXP_KR 8
-#endif
-constexpr int kR = XY_EXP_KR, kNW = 8;   // label / flip tiles: 8 warps x 8 rows = 128 x 64 (VEC 4) or 64 x 64 (VEC 2)
+constexpr int kR = 4, kNW = 8;   // label / flip tiles: TH = kR * kNW = 32 rows; 128 x 32 (VEC 4) or 64 x 32 (VEC 2)
 
 Kernels pick_kernels(uint32_t L, bool l64)
 {

@@ -219,13 +219,41 @@ __device__ __forceinline__ LabelT gfind(LabelT *lab, LabelT a)
     return a;
 }
 
+// find with path halving; the re-pointing is an atomicMin (parents only ever decrease: ancestors
+// have smaller indices), so it can never undo a concurrent min-link of the same entry.
+template <typename LabelT>
+__device__ __forceinline__ LabelT gfind_h(LabelT *lab, LabelT a)
+{
+    using A = typename AtomT<LabelT>::type;
+    LabelT r = gload(lab + a);
+    while (r != a) {
+        const LabelT g = gload(lab + r);
+        if (g == r) return r;
+        atomicMin(reinterpret_cast<A *>(lab + a), (A)g);
+        a = g;
+        r = gload(lab + a);
+    }
+    return a;
+}
+
+// a and b are most likely still roots (labels straight from k_label): try the link before any find.
+// atomicMin on lab[hi] with lo < hi is a valid step whatever hi is: if hi was a root (old == hi) it
+// is now linked into lo's component; if not, hi hangs under min(old, lo) and old, lo remain to be united.
 template <typename LabelT>
 __device__ __forceinline__ void gunion(LabelT *lab, LabelT a, LabelT b)
 {
     using A = typename AtomT<LabelT>::type;
+    if (a == b) return;
+    {
+        const LabelT hi = a > b ? a : b, lo = a > b ? b : a;
+        const LabelT old = (LabelT)atomicMin(reinterpret_cast<A *>(lab + hi), (A)lo);
+        if (old == hi || old == lo) return;
+        a = old;
+        b = lo;
+    }
     for (;;) {
-        a = gfind(lab, a);
-        b = gfind(lab, b);
+        a = gfind_h(lab, a);
+        b = gfind_h(lab, b);
         if (a == b) return;
         if (a < b) { const LabelT t = a; a = b; b = t; }
         const LabelT old = (LabelT)atomicMin(reinterpret_cast<A *>(lab + a), (A)b);

@@ -449,13 +449,8 @@ __device__ __forceinline__ void sunion_v(uint32_t *p, uint32_t a, uint32_t b)
 {
     volatile uint32_t *vp = p;
     for (;;) {
-#ifdef XY_EXP_NOHALVE
-        a = sfind_v(vp, a);
-        b = sfind_v(vp, b);
-#else
         a = sfind_h(vp, a);
         b = sfind_h(vp, b);
-#endif
         if (a == b) return;
         const uint32_t hi = a > b ? a : b, lo = a > b ? b : a;
         const uint32_t old = atomicMin(&p[hi], lo);
