@@ -413,7 +413,7 @@ k_bonds(const SweepArgs a)
 // Bonds that leave the tile are left to k_merge.
 // ---------------------------------------------------------------------------------------------
 template <int WPR, int TH>
-constexpr size_t k_label_smem_bytes() { return (size_t)(32 * WPR) * TH * 4 + (size_t)TH * WPR * 16; }
+constexpr size_t k_label_smem_bytes() { return (size_t)(32 * WPR) * TH * 4 + (size_t)TH * WPR * 12 + (size_t)(32 * WPR) * TH * 2 + 32; }
 
 __device__ __forceinline__ uint32_t nib_lo16(uint32_t v)      // low nibbles of 4 bytes -> 16 bits
 {
@@ -471,7 +471,8 @@ k_label(const SweepArgs a)
     uint32_t (*Xs)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 4);
     uint32_t (*Ss)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 4);
     uint32_t (*LLs)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 8);
-    uint32_t (*Ns)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 12);   // y bonds that unite two runs
+    uint16_t *wlist = reinterpret_cast<uint16_t *>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 12);           // per-wave lists of uniting y bonds (upper site)
+    uint32_t *wcnt = reinterpret_cast<uint32_t *>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 12 + (size_t)TW * TH * 2);   // [8] bonds in the list of wave j
 
     const uint32_t L = a.L;
     LabelT *labels = reinterpret_cast<LabelT *>(a.labels);
@@ -502,6 +503,7 @@ k_label(const SweepArgs a)
         if (LL == NONE && d <= w) LL = v;
     }
     Xs[r][w] = X; Ss[r][w] = S; LLs[r][w] = LL;
+    if (tid < 8) wcnt[tid] = 0;
     __syncthreads();
 
     // quad mapping (4 consecutive sites per thread, one row per TW/4 threads): conflict-free 16-byte
@@ -525,41 +527,42 @@ k_label(const SweepArgs a)
         *reinterpret_cast<uint4 *>(&parent[wbase + o]) = st;
     }
 
-    // ---- which y bonds unite two runs: not the redundant ones ----
+    // ---- which y bonds unite two runs: not the redundant ones.  They are sorted into one list per
+    //      union wave (below): row r is the upper row of a boundary of wave j = ctz(r + 1) + 1 ----
     {
         const int rb = (r + 1 < TH) ? r + 1 : r;
         const uint32_t J = X & Xs[rb][w] & Y;
         const uint32_t jl = __shfl_up_sync(0xffffffffu, J, 1);
-        Ns[r][w] = Y & ~((J << 1) | (w > 0 ? jl >> 31 : 0u));
+        uint32_t need = Y & ~((J << 1) | (w > 0 ? jl >> 31 : 0u));
+        if (need) {
+            const int j = __ffs(r + 1);
+            uint32_t slot = atomicAdd(&wcnt[j], (uint32_t)__popc(need)) + (uint32_t)(TW * TH - TW * (TH >> (j - 1)));
+            do {
+                const int c = __ffs(need) - 1;
+                need &= need - 1;
+                wlist[slot++] = (uint16_t)(base + c);
+            } while (need);
+        }
     }
     __syncthreads();
 
     // ---- union, in log2(TH) waves: wave j joins blocks of 2^(j-1) rows pairwise, so every wave
-    //      links roots of forests that are already flat and the trees stay shallow.  The boundary
-    //      rows of a wave are spread over ALL threads (cpi columns each).
-#pragma unroll
+    //      links roots of forests that are already flat and the trees stay shallow.  The bonds of a
+    //      wave are dealt out evenly to ALL threads from the wave's list.
+#pragma unroll 1
     for (int j = 1; (1 << j) <= TH; ++j) {
-        const int nb = TH >> j;                                // boundaries in this wave
-        const int cpi = (32 >> j) > 0 ? (32 >> j) : 1;         // columns per work item
-        const int ipb = TW / cpi;                              // items per boundary
-        if (tid < nb * ipb) {
-            const int kb = tid / ipb, it = tid - kb * ipb;
-            const int rt = (1 << (j - 1)) - 1 + (kb << j);     // upper row of the boundary
-            const int col0 = it * cpi, ww = col0 >> 5, off = col0 & 31;
-            uint32_t need = Ns[rt][ww] & (((1u << cpi) - 1u) << off);
-            const uint32_t bt = rt * TW + 32 * ww;
-            if (need) {
-                const uint32_t St = Ss[rt][ww], Sb = Ss[rt + 1][ww];
-                do {
-                    const int c = __ffs(need) - 1;
-                    need &= need - 1;
-                    const uint32_t m = (2u << c) - 1u;                             // bits <= c
-                    const uint32_t mt = St & m, mb = Sb & m;
-                    const uint32_t at = mt ? bt + 31 - __clz(mt) : LLs[rt][ww];
-                    const uint32_t ab = mb ? bt + TW + 31 - __clz(mb) : LLs[rt + 1][ww];
-                    sunion_v(parent, at, ab);
-                } while (need);
-            }
+        const uint32_t n = wcnt[j];
+        const uint16_t *lst = wlist + (TW * TH - TW * (TH >> (j - 1)));
+        const uint32_t per = (n + NT - 1) / NT, i1 = min(n, (tid + 1) * per);
+        for (uint32_t i = tid * per; i < i1; ++i) {           // contiguous share: neighbouring bonds mostly join the same runs
+            const uint32_t site = lst[i];
+            const uint32_t rt = site / TW, col = site % TW, ww = col >> 5, c = col & 31u;
+            const uint32_t m = (2u << c) - 1u;                                     // bits <= c
+            const uint32_t mt = Ss[rt][ww] & m, mb = Ss[rt + 1][ww] & m;
+            const uint32_t bt = site - c;
+            const uint32_t at = mt ? bt + 31 - __clz(mt) : LLs[rt][ww];
+            const uint32_t ab = mb ? bt + TW + 31 - __clz(mb) : LLs[rt + 1][ww];
+            sunion_v(parent, at, ab);
         }
         __syncthreads();
     }
