@@ -569,7 +569,7 @@ k_label(const SweepArgs a)
 
     // ---- flatten: ONE pass of parent[i] <- parent[parent[i]] over all entries (fixed cost, no
     //      divergence; the wave order leaves most chains at length <= 2), emit walks what is left.
-    //      In place: a racing reader sees an ancestor.
+    //      In place and without a barrier before emit: a racing reader sees an ancestor.
     {
 #pragma unroll 2
         for (int k = 0; k < TH / RPP; ++k) {
@@ -579,7 +579,6 @@ k_label(const SweepArgs a)
             p2.x = parent[p1.x]; p2.y = parent[p1.y]; p2.z = parent[p1.z]; p2.w = parent[p1.w];
             *reinterpret_cast<uint4 *>(&parent[i0]) = p2;
         }
-        __syncthreads();
     }
 
     // ---- emit: label = global index of the root; rootmask bit = "I am the tile-local root" ----
