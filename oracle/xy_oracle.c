@@ -45,6 +45,9 @@
  *                 spin wave; the paper's Table I row L=64.
  *   observe     : independent numpy evaluation with math.fsum.
  *   pcc         : injected monotone observable; paper's beta_KT(64).
+ *   fourier     : numpy FFT of the spin field; plane wave and uniform closed forms;
+ *                 Eq. 8 inverts the Ornstein-Zernike form exactly; xi_2nd/L of the
+ *                 paper's Table I row L=64.
  * No function here is "parity unpinned".
  */
 #include <math.h>
@@ -367,6 +370,50 @@ void xyo_observe(const float *theta, uint32_t L32, xyo_obs *o)
     o->Cx = nval(&cx); o->Sx = nval(&sx);
     o->Cy = nval(&cy); o->Sy = nval(&sy);
     o->E = -(o->Cx + o->Cy);
+}
+
+/* ------------------------------------------------------------------------- */
+/* O9 (next row after the hot path: second-moment correlation length,          */
+/* PAPER.md:100-107 Eq. 8-9).  Structure-factor sums at the smallest wave      */
+/* vectors k = 2 pi / L along x and along y, every term in fp64:               */
+/*   F[0..3] = sum_r ( cos th cos kx, cos th sin kx, sin th cos kx, sin th sin kx ) */
+/*   F[4..7] = the same with ky in place of kx,   phase = 2pi64 * (x / L).     */
+/* Then sum_r s(r) e^{ikr} has |.|^2 = F0^2 + F1^2 + F2^2 + F3^2 (x direction). */
+/* Eq. 9 as printed squares the average; the standard estimator, used here and */
+/* consistent with chi(0) = N <m^2> of Eq. 10, averages the square:            */
+/*   chi(k) = < |sum_r s(r) e^{ikr}|^2 > / N   (reading G21).        */
+/* ------------------------------------------------------------------------- */
+void xyo_fourier(const float *theta, uint32_t L32, double F[8])
+{
+    uint64_t L = L32;
+    nsum f[8];
+    for (int k = 0; k < 8; ++k) { f[k].s = 0.0; f[k].c = 0.0; }
+    for (uint64_t y = 0; y < L; ++y) {
+        double ay = XYO_TWO_PI * ((double)y / (double)L);
+        double cy = cos(ay), sy = sin(ay);
+        for (uint64_t x = 0; x < L; ++x) {
+            double ax = XYO_TWO_PI * ((double)x / (double)L);
+            double cx = cos(ax), sx = sin(ax);
+            double ti = (double)theta[y * L + x];
+            double c = cos(ti), s = sin(ti);
+            nadd(&f[0], c * cx); nadd(&f[1], c * sx); nadd(&f[2], s * cx); nadd(&f[3], s * sx);
+            nadd(&f[4], c * cy); nadd(&f[5], c * sy); nadd(&f[6], s * cy); nadd(&f[7], s * sy);
+        }
+    }
+    for (int k = 0; k < 8; ++k) F[k] = nval(&f[k]);
+}
+
+/* |sum_r s(r) e^{ikr}|^2 / N of ONE configuration from its four sums          */
+double xyo_sk(const double F4[4], uint32_t L32)
+{
+    double N = (double)L32 * (double)L32;
+    return (F4[0] * F4[0] + F4[1] * F4[1] + F4[2] * F4[2] + F4[3] * F4[3]) / N;
+}
+
+/* Eq. 8: xi_2nd(L) = sqrt(chi(0)/chi(2pi/L) - 1) / (2 sin(pi/L))              */
+double xyo_xi2nd(double chi0, double chik, uint32_t L32)
+{
+    return sqrt(chi0 / chik - 1.0) / (2.0 * sin(XYO_PI / (double)L32));
 }
 
 /* ------------------------------------------------------------------------- */

@@ -86,6 +86,9 @@ _reflect = _sig("xyo_reflect", C.c_float, [C.c_float, C.c_double])
 _flip_sites = _sig("xyo_flip_sites", None, [f32p, C.c_uint64, C.c_double, u8p])
 _flip = _sig("xyo_flip", C.c_uint64, [f32p, C.c_uint32, i64p, C.c_double, C.c_uint64, C.c_uint64])
 _observe = _sig("xyo_observe", None, [f32p, C.c_uint32, C.POINTER(Obs)])
+_fourier = _sig("xyo_fourier", None, [f32p, C.c_uint32, C.POINTER(C.c_double)])
+_sk = _sig("xyo_sk", C.c_double, [C.POINTER(C.c_double), C.c_uint32])
+_xi2nd = _sig("xyo_xi2nd", C.c_double, [C.c_double, C.c_double, C.c_uint32])
 _sweep = _sig("xyo_sweep", C.c_int,
               [f32p, C.c_uint32, C.c_uint64, C.c_uint64, C.c_double, C.c_int, C.c_double,
                u8p, i64p, C.POINTER(Obs)])
@@ -206,6 +209,24 @@ def observe(theta, L):
     o = Obs()
     _observe(theta, L, C.byref(o))
     return o
+
+
+def fourier(theta, L):
+    """The 8 structure-factor sums at k = 2 pi / L (x: F[0:4], y: F[4:8]) of one configuration."""
+    F = (C.c_double * 8)()
+    _fourier(theta, L, F)
+    return np.array(F[:], dtype=np.float64)
+
+
+def sk(F4, L):
+    """|sum_r s(r) e^{ikr}|^2 / N from the four sums of one direction."""
+    a = (C.c_double * 4)(*[float(v) for v in F4])
+    return _sk(a, L)
+
+
+def xi2nd(chi0, chik, L):
+    """PAPER.md:102 Eq. 8."""
+    return _xi2nd(chi0, chik, L)
 
 
 def sweep(theta, L, seed, t, beta, fix_phi=None):
