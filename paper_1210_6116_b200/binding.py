@@ -13,6 +13,7 @@ _LIB_PATH = os.path.join(_HERE, "libxy_b200.so")
 
 INIT_COLD, INIT_HOT = 0, 1
 FLAG_LABELS64 = 1
+FLAG_FOURIER = 2
 
 
 class XYError(RuntimeError):
@@ -52,6 +53,14 @@ OBS_DTYPE = np.dtype([("sweep", "<u8"), ("beta", "<f8"), ("E", "<f8"), ("Mx", "<
 assert OBS_DTYPE.itemsize == C.sizeof(Obs)
 
 
+class Fourier(C.Structure):
+    _fields_ = [("sweep", C.c_uint64), ("Fx", C.c_double * 4), ("Fy", C.c_double * 4)]
+
+
+FOURIER_DTYPE = np.dtype([("sweep", "<u8"), ("Fx", "<f8", (4,)), ("Fy", "<f8", (4,))])
+assert FOURIER_DTYPE.itemsize == C.sizeof(Fourier)
+
+
 class PccSchedule(C.Structure):
     _fields_ = [("n_sweeps", C.c_uint64), ("discard", C.c_uint64),
                 ("window", C.c_uint32), ("dirs", C.c_uint32),
@@ -80,6 +89,8 @@ _SIGS = {
     "xy_get_labels": [_vp, _vp, C.c_size_t],
     "xy_get_bonds": [_vp, _vp, C.c_size_t],
     "xy_get_series": [_vp, _vp, C.c_uint64, C.c_uint64],
+    "xy_measure_fourier": [_vp, C.POINTER(Fourier)],
+    "xy_get_fourier_series": [_vp, _vp, C.c_uint64, C.c_uint64],
     "xy_series_capacity": [_vp, C.POINTER(C.c_uint64)],
     "xy_get_sweep": [_vp, C.POINTER(C.c_uint64)],
     "xy_set_sweep": [_vp, C.c_uint64],
@@ -195,6 +206,17 @@ class XYState:
     def get_bonds(self):
         out = np.empty(self.N, np.uint8)
         _check(_lib.xy_get_bonds(self._h, out.ctypes.data, self.N))
+        return out
+
+    def measure_fourier(self):
+        """The 8 structure-factor sums of the current configuration (needs FLAG_FOURIER): array [8] = Fx, Fy."""
+        f = Fourier()
+        _check(_lib.xy_measure_fourier(self._h, C.byref(f)))
+        return np.array(list(f.Fx) + list(f.Fy), dtype=np.float64)
+
+    def get_fourier_series(self, first, count):
+        out = np.zeros(count, FOURIER_DTYPE)
+        _check(_lib.xy_get_fourier_series(self._h, out.ctypes.data, first, count))
         return out
 
     def get_series(self, first, count):

@@ -45,7 +45,7 @@ constexpr size_t kStageBytes = 64u << 20;  // staging buffer of the debug getter
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-    size_t theta, labels, bonds, rootmask, partials, ring, ctl, tab, total;
+    size_t theta, labels, bonds, rootmask, partials, ring, fring, ctl, tab, total;
 };
 
 Layout make_layout(uint32_t L, uint32_t flags)
@@ -60,6 +60,7 @@ Layout make_layout(uint32_t L, uint32_t flags)
     o.rootmask = off; off = align_up(off + N / 8, 256);
     o.partials = off; off = align_up(off + (size_t)kMaxGrid * kPartialStride * 8, 256);
     o.ring = off;     off = align_up(off + (size_t)kRingCap * sizeof(xy_obs), 256);
+    o.fring = off;    off = align_up(off + ((flags & XY_FLAG_FOURIER) ? (size_t)kRingCap * sizeof(xy_fourier) : 0), 256);
     o.ctl = off;      off = align_up(off + sizeof(DevCtl), 256);
     o.tab = off;      off = align_up(off + (size_t)(kTabN + 1) * sizeof(double2), 256);
     o.total = off;
@@ -68,11 +69,11 @@ Layout make_layout(uint32_t L, uint32_t flags)
 
 // One set of launchers per (tile geometry, label width).
 struct Kernels {
-    void (*bonds)(const SweepArgs &, bool obs_only, int grid, cudaStream_t);
+    void (*bonds)(const SweepArgs &, bool obs_only, bool fourier, int grid, cudaStream_t);
     void (*label)(const SweepArgs &, cudaStream_t);
     void (*merge)(const SweepArgs &, cudaStream_t);
     void (*flip)(const SweepArgs &, int grid, cudaStream_t);
-    int (*occupancy)(int *bonds_sweep, int *bonds_obs, int *fl);
+    int (*occupancy)(bool fourier, int *bonds_sweep, int *bonds_obs, int *fl);
     int tw, th, rs;
 };
 
@@ -81,10 +82,15 @@ constexpr int kBondsWarps = 4;   // warps per CTA in k_bonds
 
 template <int VEC, int R, int NW, typename LabelT>
 struct KS {
-    static void bonds(const SweepArgs &a, bool obs_only, int grid, cudaStream_t st)
+    static void bonds(const SweepArgs &a, bool obs_only, bool fourier, int grid, cudaStream_t st)
     {
-        if (obs_only) k_bonds<VEC, kRS, false><<<grid, kBondsWarps * 32, 0, st>>>(a);
-        else k_bonds<VEC, kRS, true><<<grid, kBondsWarps * 32, 0, st>>>(a);
+        if (fourier) {
+            if (obs_only) k_bonds<VEC, kRS, false, true><<<grid, kBondsWarps * 32, 0, st>>>(a);
+            else k_bonds<VEC, kRS, true, true><<<grid, kBondsWarps * 32, 0, st>>>(a);
+        } else {
+            if (obs_only) k_bonds<VEC, kRS, false, false><<<grid, kBondsWarps * 32, 0, st>>>(a);
+            else k_bonds<VEC, kRS, true, false><<<grid, kBondsWarps * 32, 0, st>>>(a);
+        }
     }
     static void label(const SweepArgs &a, cudaStream_t st)
     {
@@ -108,12 +114,14 @@ struct KS {
         (void)grid;
         k_flip<VEC, R * NW, LabelT><<<a.ntiles, VEC * R * NW, 0, st>>>(a);
     }
-    static int occupancy(int *bonds_sweep, int *bonds_obs, int *fl)
+    static int occupancy(bool fourier, int *bonds_sweep, int *bonds_obs, int *fl)
     {
         cudaError_t e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_sweep, k_bonds<VEC, kRS, true>, kBondsWarps * 32, 0);
+        if (fourier) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_sweep, k_bonds<VEC, kRS, true, true>, kBondsWarps * 32, 0);
+        else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_sweep, k_bonds<VEC, kRS, true, false>, kBondsWarps * 32, 0);
         if (e != cudaSuccess) return (int)e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_obs, k_bonds<VEC, kRS, false>, kBondsWarps * 32, 0);
+        if (fourier) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_obs, k_bonds<VEC, kRS, false, true>, kBondsWarps * 32, 0);
+        else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_obs, k_bonds<VEC, kRS, false, false>, kBondsWarps * 32, 0);
         if (e != cudaSuccess) return (int)e;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(fl, k_flip<VEC, R * NW, LabelT>, VEC * R * NW, 0);
         return (int)e;
@@ -235,6 +243,8 @@ struct xy_state {
     DevCtl *ctl() const { return reinterpret_cast<DevCtl *>(ws + lay.ctl); }
     double2 *tab() const { return reinterpret_cast<double2 *>(ws + lay.tab); }
     bool l64() const { return (flags & XY_FLAG_LABELS64) != 0; }
+    bool fourier() const { return (flags & XY_FLAG_FOURIER) != 0; }
+    xy_fourier *fring() const { return reinterpret_cast<xy_fourier *>(ws + lay.fring); }
 };
 
 namespace {
@@ -284,6 +294,12 @@ SweepArgs base_args(const xy_state *s)
     }
     a.t = (uint32_t)s->T;
     a.sincos_tab = s->tab();
+    a.fring = s->fring();
+    {
+        const long double ang = 6.283185307179586476925286766559L / (long double)s->L;
+        a.ck1 = (double)cosl(ang);
+        a.sk1 = (double)sinl(ang);
+    }
     return a;
 }
 
@@ -319,7 +335,7 @@ int ensure_obs(xy_state *s, int feed_pcc)
     SweepArgs a = base_args(s);
     a.obs_fill = 1;
     a.feed_pcc = feed_pcc;
-    s->ker.bonds(a, true, s->grid_bonds, s->stream);
+    s->ker.bonds(a, true, s->fourier(), s->grid_bonds, s->stream);
     CUDA_TRY(cudaGetLastError());
     s->launches += 1;
     s->obs_valid_T = s->T;
@@ -371,7 +387,7 @@ int enqueue_sweep(xy_state *s, double beta, int beta_from_ctl, int feed_pcc)
             if (int rc = timing_flush(s)) return rc;
         if (int rc = timing_mark(s)) return rc;
     }
-    s->ker.bonds(a, false, s->grid_bonds, s->stream);
+    s->ker.bonds(a, false, s->fourier(), s->grid_bonds, s->stream);
     if (s->timing) if (int rc = timing_mark(s)) return rc;
     s->ker.label(a, s->stream);
     if (s->timing) if (int rc = timing_mark(s)) return rc;
@@ -399,7 +415,7 @@ int xy_workspace_bytes(uint32_t L, uint32_t flags, size_t *nbytes)
 {
     if (!nbytes) return fail(XY_ERR_ARG, "nbytes is NULL");
     if (int rc = check_L(L)) return rc;
-    if (flags & ~(uint32_t)XY_FLAG_LABELS64) return fail(XY_ERR_ARG, "unknown flags 0x%x", flags);
+    if (flags & ~(uint32_t)(XY_FLAG_LABELS64 | XY_FLAG_FOURIER)) return fail(XY_ERR_ARG, "unknown flags 0x%x", flags);
     *nbytes = make_layout(L, flags).total;
     return XY_OK;
 }
@@ -410,7 +426,7 @@ int xy_create_ex(xy_state **out, uint32_t L, uint64_t seed, int init, uint32_t f
     *out = nullptr;
     if (int rc = check_L(L)) return rc;
     if (init != XY_INIT_COLD && init != XY_INIT_HOT) return fail(XY_ERR_ARG, "init=%d unknown", init);
-    if (flags & ~(uint32_t)XY_FLAG_LABELS64) return fail(XY_ERR_ARG, "unknown flags 0x%x", flags);
+    if (flags & ~(uint32_t)(XY_FLAG_LABELS64 | XY_FLAG_FOURIER)) return fail(XY_ERR_ARG, "unknown flags 0x%x", flags);
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
         return fail(XY_ERR_CUDA, "no CUDA device: this library has no CPU fallback");
@@ -439,7 +455,7 @@ int xy_create_ex(xy_state **out, uint32_t L, uint64_t seed, int init, uint32_t f
         s->owns_ws = true;
     }
     int bs = 0, bo = 0, fl = 0, sms = 0;
-    cudaError_t e = (cudaError_t)s->ker.occupancy(&bs, &bo, &fl);
+    cudaError_t e = (cudaError_t)s->ker.occupancy(s->fourier(), &bs, &bo, &fl);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device);
     if (e != cudaSuccess || bs < 1 || bo < 1 || fl < 1) {
         if (s->owns_ws) cudaFree(s->ws);
@@ -708,6 +724,40 @@ int xy_get_series(xy_state *s, xy_obs *host, uint64_t first, uint64_t count)
         uint64_t run = kRingCap - slot;
         if (run > count - done) run = count - done;
         CUDA_TRY(cudaMemcpyAsync(host + done, s->ring() + slot, run * sizeof(xy_obs), cudaMemcpyDeviceToHost, s->stream));
+        done += run;
+    }
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    return XY_OK;
+}
+
+int xy_measure_fourier(xy_state *s, xy_fourier *out)
+{
+    if (!s || !out) return fail(XY_ERR_ARG, "NULL argument");
+    if (!s->fourier()) return fail(XY_ERR_STATE, "state was created without XY_FLAG_FOURIER");
+    DeviceGuard g(s->device);
+    if (int rc = ensure_obs(s, 0)) return rc;
+    CUDA_TRY(cudaMemcpyAsync(out, s->fring() + (s->T % kRingCap), sizeof(xy_fourier), cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    return XY_OK;
+}
+
+int xy_get_fourier_series(xy_state *s, xy_fourier *host, uint64_t first, uint64_t count)
+{
+    if (!s || (!host && count)) return fail(XY_ERR_ARG, "NULL argument");
+    if (!s->fourier()) return fail(XY_ERR_STATE, "state was created without XY_FLAG_FOURIER");
+    if (count == 0) return XY_OK;
+    if (first < s->oldest_T || first + count - 1 > s->T)
+        return fail(XY_ERR_ARG, "records %llu..%llu not in the ring (holds %llu..%llu)", (unsigned long long)first,
+                    (unsigned long long)(first + count - 1), (unsigned long long)s->oldest_T, (unsigned long long)s->T);
+    DeviceGuard g(s->device);
+    if (first + count - 1 == s->T)
+        if (int rc = ensure_obs(s, 0)) return rc;
+    uint64_t done = 0;
+    while (done < count) {
+        const uint64_t slot = (first + done) % kRingCap;
+        uint64_t run = kRingCap - slot;
+        if (run > count - done) run = count - done;
+        CUDA_TRY(cudaMemcpyAsync(host + done, s->fring() + slot, run * sizeof(xy_fourier), cudaMemcpyDeviceToHost, s->stream));
         done += run;
     }
     CUDA_TRY(cudaStreamSynchronize(s->stream));

@@ -21,7 +21,7 @@
 
 namespace xy {
 
-constexpr int kPartialStride = 8;          // doubles per CTA partial record
+constexpr int kPartialStride = 16;         // doubles per CTA partial record: 14 sums + 2 counts
 
 // Device-resident control block: PCC controller (O8) + counters.
 struct DevCtl {
@@ -65,7 +65,9 @@ struct SweepArgs {
     int          obs_fill;        // 1: finalize writes the observables of the incoming state into ring[T]
     double       beta;
     double       phi, cphi, sphi, A;
-    const double2 *sincos_tab;    // [257] (cos, sin)(2 pi k / 256), host-computed
+    const double2 *sincos_tab;    // [kTabN + 1] (cos, sin)(2 pi k / kTabN), host-computed
+    double       ck1, sk1;        // (cos, sin)(2 pi / L)
+    xy_fourier  *fring;           // ring of structure-factor records (XY_FLAG_FOURIER), else unused
 };
 
 
@@ -160,18 +162,23 @@ __device__ __forceinline__ void sincos_tab(float theta, const double2 *tab, doub
     s = __fma_rn(cs.x, sx, __fma_rn(cs.y, dc, cs.y));
 }
 
-template <int VEC, int RS, bool kBonds>
-__global__ void __launch_bounds__(128, 4)
+// kFourier: also reduce the 8 structure-factor sums at k = 2 pi / L (x and y direction) of the
+// incoming configuration (Eq. 8-9): per-column sums of (cos, sin) live in registers
+// for the 32 rows of a strip and meet e^{ik x} once per strip; per-row sums meet e^{ik y} once per row.
+template <int VEC, int RS, bool kBonds, bool kFourier>
+__global__ void __launch_bounds__(128, kFourier ? 3 : 4)
 k_bonds(const SweepArgs a)
 {
     constexpr int NW = 4;
+    constexpr int NS = kFourier ? 14 : 6;      // fp64 sums per thread / warp / CTA
     constexpr int TW = 32 * VEC;
     static_assert(RS <= 32, "halo column is computed by one lane per row");
 
     __shared__ double2 tab[kTabN + 1];
     __shared__ double h_c[NW][RS], h_s[NW][RS];
     __shared__ float h_t[NW][RS], h_g[NW][RS];
-    __shared__ double red[NW][6];
+    __shared__ double red[NW][NS];
+    __shared__ double2 h_ky[kFourier ? NW : 1][RS];      // (cos, sin)(2 pi y / L) of the strip's rows
     __shared__ unsigned long long redc[NW][2];
     __shared__ bool is_last;
 
@@ -191,6 +198,7 @@ k_bonds(const SweepArgs a)
     const double cphi = a.cphi, sphi = a.sphi;
 
     double aMx = 0, aMy = 0, aCx = 0, aSx = 0, aCy = 0, aSy = 0;
+    double aF[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // kFourier: Fx[0..3], Fy[0..3]
     uint32_t nbx = 0, nby = 0;
 
     const uint32_t strips_x = L / TW;
@@ -211,8 +219,16 @@ k_bonds(const SweepArgs a)
             h_c[warp][lane] = c;
             h_s[warp][lane] = s;
             h_g[warp][lane] = __double2float_rn(__fma_rn(c, cphi, s * sphi));
+            if constexpr (kFourier) {
+                double sk, ck;
+                sincospi(2.0 * (double)(y0 + lane) / (double)L, &sk, &ck);
+                h_ky[warp][lane] = make_double2(ck, sk);
+            }
         }
         __syncwarp();
+        double colC[VEC], colS[VEC];             // kFourier: column sums over the strip's rows
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) { colC[v] = 0.0; colS[v] = 0.0; }
 
         // two register sets (A, B) alternate as "row being finished" and "row below": no copies
         float tA[VEC], tB[VEC], gA[VEC], gB[VEC];
@@ -262,8 +278,8 @@ k_bonds(const SweepArgs a)
             for (int v = VEC - 1; v >= 0; --v) {
                 const double c2 = (v + 1 < VEC) ? pc[(v + 1) % VEC] : cn;
                 const double s2 = (v + 1 < VEC) ? ps[(v + 1) % VEC] : sn;
-                aMx += pc[v];
-                aMy += ps[v];
+                if constexpr (kFourier) { colC[v] += pc[v]; colS[v] += ps[v]; }
+                else { aMx += pc[v]; aMy += ps[v]; }
                 aCx = __fma_rn(pc[v], c2, aCx);
                 aCx = __fma_rn(ps[v], s2, aCx);
                 aSx = __fma_rn(ps[v], c2, aSx);
@@ -281,6 +297,14 @@ k_bonds(const SweepArgs a)
                     xn = __funnelshift_l(__float_as_uint(dx[v]), xn, 1);      // (xn << 1) | sign(dx): active iff d < 0
                     yn = __funnelshift_l(__float_as_uint(dy[v]), yn, 1);
                 }
+            }
+            if constexpr (kFourier) {
+                double rc = pc[0], rs = ps[0];
+#pragma unroll
+                for (int v = 1; v < VEC; ++v) { rc += pc[v]; rs += ps[v]; }
+                const double2 ky = h_ky[warp][r - 1];
+                aF[4] = __fma_rn(rc, ky.x, aF[4]); aF[5] = __fma_rn(rc, ky.y, aF[5]);
+                aF[6] = __fma_rn(rs, ky.x, aF[6]); aF[7] = __fma_rn(rs, ky.y, aF[7]);
             }
             if constexpr (kBonds) {
                 if (dmin <= kFilterDelta) {              // rare: some decision of this lane is too close to call
@@ -320,29 +344,49 @@ k_bonds(const SweepArgs a)
             step(r, tA, cA, sA, gA, tB, cB, sB, gB);
             step(r + 1, tB, cB, sB, gB, tA, cA, sA, gA);
         }
+        if constexpr (kFourier) {
+            double sk, ck;
+            sincospi(2.0 * (double)xl / (double)L, &sk, &ck);
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) {
+                aMx += colC[v]; aMy += colS[v];
+                aF[0] = __fma_rn(colC[v], ck, aF[0]); aF[1] = __fma_rn(colC[v], sk, aF[1]);
+                aF[2] = __fma_rn(colS[v], ck, aF[2]); aF[3] = __fma_rn(colS[v], sk, aF[3]);
+                const double cn = __fma_rn(ck, a.ck1, -sk * a.sk1);      // next column: rotate by 2 pi / L
+                sk = __fma_rn(sk, a.ck1, ck * a.sk1);
+                ck = cn;
+            }
+        }
     }
 
     // ---- per-CTA partial sums, fixed tree ----
-    aMx = warp_sum(aMx); aMy = warp_sum(aMy); aCx = warp_sum(aCx);
-    aSx = warp_sum(aSx); aCy = warp_sum(aCy); aSy = warp_sum(aSy);
+    double acc[NS];
+    acc[0] = aMx; acc[1] = aMy; acc[2] = aCx; acc[3] = aSx; acc[4] = aCy; acc[5] = aSy;
+    if constexpr (kFourier) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) acc[6 + k] = aF[k];
+    }
+#pragma unroll
+    for (int k = 0; k < NS; ++k) acc[k] = warp_sum(acc[k]);
     unsigned long long cbx = warp_sum_u64(nbx), cby = warp_sum_u64(nby);
     if (lane == 0) {
-        red[warp][0] = aMx; red[warp][1] = aMy; red[warp][2] = aCx;
-        red[warp][3] = aSx; red[warp][4] = aCy; red[warp][5] = aSy;
+#pragma unroll
+        for (int k = 0; k < NS; ++k) red[warp][k] = acc[k];
         redc[warp][0] = cbx; redc[warp][1] = cby;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        double acc[6] = {0, 0, 0, 0, 0, 0};
+        double tot[NS];
+        for (int k = 0; k < NS; ++k) tot[k] = 0.0;
         unsigned long long c0 = 0, c1 = 0;
         for (int w = 0; w < NW; ++w) {
-            for (int k = 0; k < 6; ++k) acc[k] += red[w][k];
+            for (int k = 0; k < NS; ++k) tot[k] += red[w][k];
             c0 += redc[w][0]; c1 += redc[w][1];
         }
         double *p = a.partials + (size_t)blockIdx.x * kPartialStride;
-        for (int k = 0; k < 6; ++k) p[k] = acc[k];
-        p[6] = __longlong_as_double((long long)c0);
-        p[7] = __longlong_as_double((long long)c1);
+        for (int k = 0; k < NS; ++k) p[k] = tot[k];
+        p[14] = __longlong_as_double((long long)c0);
+        p[15] = __longlong_as_double((long long)c1);
         __threadfence();
         const unsigned int ticket = atomicAdd(&a.ctl->ticket, 1u);
         is_last = (ticket == gridDim.x - 1);
@@ -353,28 +397,36 @@ k_bonds(const SweepArgs a)
     // ---- finalize (S8): the last CTA reduces the partials in a fixed order ----
     __threadfence();
     {
-        double acc[6] = {0, 0, 0, 0, 0, 0};
+        for (int k = 0; k < NS; ++k) acc[k] = 0.0;
         unsigned long long c0 = 0, c1 = 0;
         for (uint32_t b = threadIdx.x; b < gridDim.x; b += blockDim.x) {
             const double *p = a.partials + (size_t)b * kPartialStride;
-            for (int k = 0; k < 6; ++k) acc[k] += __ldcg(p + k);
-            c0 += (unsigned long long)__double_as_longlong(__ldcg(p + 6));
-            c1 += (unsigned long long)__double_as_longlong(__ldcg(p + 7));
+            for (int k = 0; k < NS; ++k) acc[k] += __ldcg(p + k);
+            c0 += (unsigned long long)__double_as_longlong(__ldcg(p + 14));
+            c1 += (unsigned long long)__double_as_longlong(__ldcg(p + 15));
         }
-        for (int k = 0; k < 6; ++k) acc[k] = warp_sum(acc[k]);
+        for (int k = 0; k < NS; ++k) acc[k] = warp_sum(acc[k]);
         c0 = warp_sum_u64(c0); c1 = warp_sum_u64(c1);
         __syncthreads();
         if (lane == 0) {
-            for (int k = 0; k < 6; ++k) red[warp][k] = acc[k];
+            for (int k = 0; k < NS; ++k) red[warp][k] = acc[k];
             redc[warp][0] = c0; redc[warp][1] = c1;
         }
         __syncthreads();
         if (threadIdx.x == 0) {
-            double tot[6] = {0, 0, 0, 0, 0, 0};
+            double tot[NS];
+            for (int k = 0; k < NS; ++k) tot[k] = 0.0;
             unsigned long long b0 = 0, b1 = 0;
             for (int w = 0; w < NW; ++w) {
-                for (int k = 0; k < 6; ++k) tot[k] += red[w][k];
+                for (int k = 0; k < NS; ++k) tot[k] += red[w][k];
                 b0 += redc[w][0]; b1 += redc[w][1];
+            }
+            if constexpr (kFourier) {
+                if (a.obs_fill) {
+                    xy_fourier *f = a.fring + (a.t % a.ring_cap);   // record of T = t (the incoming state)
+                    f->sweep = (uint64_t)a.t;
+                    for (int k = 0; k < 4; ++k) { f->Fx[k] = tot[6 + k]; f->Fy[k] = tot[10 + k]; }
+                }
             }
             const double N = (double)L * (double)L;
             if (a.obs_fill) {
