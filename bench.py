@@ -216,6 +216,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4", choices=sorted(WORKLOADS))
     ap.add_argument("--labels64", action="store_true", help="hold labels as 64-bit words")
+    ap.add_argument("--fourier", action="store_true",
+                    help="also reduce the structure-factor sums of every sweep (xi_2nd; XY_FLAG_FOURIER)")
     ap.add_argument("--e2e-steps", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -240,7 +242,7 @@ def main():
 
     cfg_idx, L, init, seed, beta, therm = WORKLOADS[args.workload]
     N = L * L
-    flags = xy.FLAG_LABELS64 if args.labels64 else 0
+    flags = (xy.FLAG_LABELS64 if args.labels64 else 0) | (xy.FLAG_FOURIER if args.fourier else 0)
     label_bytes = 8 if args.labels64 else 4
     tw, th = (128, 32) if L % 128 == 0 else (64, 32)
     K, W = args.steps, max(args.warmup, 0)
@@ -332,7 +334,7 @@ def main():
             "config": {"workload": f"BASELINE config {cfg_idx + 1 if cfg_idx is not None else '-'} ({args.workload}): "
                                    f"2D XY L={L} periodic, {init} start seed {seed}, beta={beta}, "
                                    f"{therm} thermalisation sweeps untimed",
-                       "L": L, "beta": beta, "label_bytes": label_bytes, "tile": f"{tw}x{th}",
+                       "L": L, "beta": beta, "label_bytes": label_bytes, "fourier_sums": bool(args.fourier), "tile": f"{tw}x{th}",
                        "replicas": world, "parallelism": "replicas only (the path does not shard)",
                        "l2": "working set %.2f GiB per sweep >> 126 MB L2, no flush needed" % ((4 + label_bytes + 0.25) * N / 2 ** 30)
                        if (4 + label_bytes) * N > 4 * 126e6 else "working set fits L2: number is NOT an HBM measurement"},
