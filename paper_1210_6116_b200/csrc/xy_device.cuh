@@ -164,8 +164,9 @@ __device__ __forceinline__ float reflect(float theta, double A)
 {
     double d = __dsub_rn(A, (double)theta);
     // "while (d < 0) d += 2pi": A >= 0 and theta <= fl32(2pi) < 2 * 2pi64 give d > -2 * 2pi64, so twice is enough
-    if (d < 0.0) d = __dadd_rn(d, kTwoPi);
-    if (d < 0.0) d = __dadd_rn(d, kTwoPi);
+    // the sign is read from the high word (integer compare instead of an fp64 one; A - theta is never -0.0)
+    if (__double2hiint(d) < 0) d = __dadd_rn(d, kTwoPi);
+    if (__double2hiint(d) < 0) d = __dadd_rn(d, kTwoPi);
     return __double2float_rn(d);
 }
 

@@ -824,21 +824,23 @@ k_flip(const SweepArgs a)
         const float th[4] = {t4.x, t4.y, t4.z, t4.w};
         LabelT lab[4];
         load_labels(i, lab);
-        float out[4];
-        bool any = false;
+        uint32_t coins = 0;
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
-            uint32_t loc = loc0 + v;
-            if (!((rb >> (4 * k + v)) & 1u)) {
-                const uint32_t d = (uint32_t)(lab[v] - gbase);          // r*L + c, < TH*L <= 2^22
-                const uint32_t rr = __umulhi(d, a.Ldiv_mul) >> a.Ldiv_shift;
-                loc = d - rr * Lm;
-            }
-            const bool coin = (cbits[loc >> 5] >> (loc & 31u)) & 1u;
-            out[v] = coin ? reflect(th[v], a.A) : th[v];
-            any |= coin;
+            const uint32_t d = (uint32_t)(lab[v] - gbase);              // r*L + c, < TH*L <= 2^22
+            const uint32_t rr = __umulhi(d, a.Ldiv_mul) >> a.Ldiv_shift;
+            const uint32_t loc = ((rb >> (4 * k + v)) & 1u) ? loc0 + v : d - rr * Lm;
+            coins |= ((cbits[loc >> 5] >> (loc & 31u)) & 1u) << v;
         }
-        if (any) *reinterpret_cast<float4 *>(a.theta + i) = make_float4(out[0], out[1], out[2], out[3]);
+        if (coins) {                                                    // one branch per 4 sites; straight-line inside
+            float out[4];
+#pragma unroll
+            for (int v = 0; v < 4; ++v) {
+                const float rf = reflect(th[v], a.A);
+                out[v] = ((coins >> v) & 1u) ? rf : th[v];
+            }
+            *reinterpret_cast<float4 *>(a.theta + i) = make_float4(out[0], out[1], out[2], out[3]);
+        }
     }
 
     unsigned long long c = warp_sum_u64(ncl);
