@@ -465,7 +465,7 @@ k_bonds(const SweepArgs a)
 // Bonds that leave the tile are left to k_merge.
 // ---------------------------------------------------------------------------------------------
 template <int WPR, int TH>
-constexpr size_t k_label_smem_bytes() { return (size_t)(32 * WPR) * TH * 4 + (size_t)TH * WPR * 12 + (size_t)(32 * WPR) * TH * 2 + 32; }
+constexpr size_t k_label_smem_bytes() { return (size_t)(32 * WPR) * TH * 4 + (size_t)TH * WPR * 12 + (size_t)(32 * WPR) * TH + 32; }
 
 __device__ __forceinline__ uint32_t nib_lo16(uint32_t v)      // low nibbles of 4 bytes -> 16 bits
 {
@@ -517,6 +517,7 @@ __global__ void __launch_bounds__(WPR * TH, 1536 / (WPR * TH))
 k_label(const SweepArgs a)
 {
     constexpr int TW = 32 * WPR, NT = WPR * TH;
+    constexpr uint32_t LCAP = TW * TH / 2;           // entries of the wave lists: half the worst case (every y bond uniting)
     constexpr uint32_t NONE = 0xffffffffu;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     uint32_t *parent = reinterpret_cast<uint32_t *>(smem_raw);                       // [TW*TH]
@@ -524,7 +525,7 @@ k_label(const SweepArgs a)
     uint32_t (*Ss)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 4);
     uint32_t (*LLs)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 8);
     uint16_t *wlist = reinterpret_cast<uint16_t *>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 12);           // per-wave lists of uniting y bonds (upper site)
-    uint32_t *wcnt = reinterpret_cast<uint32_t *>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 12 + (size_t)TW * TH * 2);   // [8] bonds in the list of wave j
+    uint32_t *wcnt = reinterpret_cast<uint32_t *>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 12 + (size_t)TW * TH);   // [8] bonds in the list of wave j
 
     const uint32_t L = a.L;
     LabelT *labels = reinterpret_cast<LabelT *>(a.labels);
@@ -579,21 +580,24 @@ k_label(const SweepArgs a)
         *reinterpret_cast<uint4 *>(&parent[wbase + o]) = st;
     }
 
+    uint32_t need = 0;
+    int myj = 0;
     // ---- which y bonds unite two runs: not the redundant ones.  They are sorted into one list per
     //      union wave (below): row r is the upper row of a boundary of wave j = ctz(r + 1) + 1 ----
     {
         const int rb = (r + 1 < TH) ? r + 1 : r;
         const uint32_t J = X & Xs[rb][w] & Y;
         const uint32_t jl = __shfl_up_sync(0xffffffffu, J, 1);
-        uint32_t need = Y & ~((J << 1) | (w > 0 ? jl >> 31 : 0u));
+        need = Y & ~((J << 1) | (w > 0 ? jl >> 31 : 0u));
         if (need) {
-            const int j = __ffs(r + 1);
-            uint32_t slot = atomicAdd(&wcnt[j], (uint32_t)__popc(need)) + (uint32_t)(TW * TH - TW * (TH >> (j - 1)));
-            do {
+            myj = __ffs(r + 1);
+            const uint32_t cap = LCAP >> myj, off = LCAP - (LCAP >> (myj - 1));
+            uint32_t slot = atomicAdd(&wcnt[myj], (uint32_t)__popc(need));
+            while (need && slot < cap) {             // what does not fit (lists hold half the worst case) stays with this thread
                 const int c = __ffs(need) - 1;
                 need &= need - 1;
-                wlist[slot++] = (uint16_t)(base + c);
-            } while (need);
+                wlist[off + slot++] = (uint16_t)(base + c);
+            }
         }
     }
     __syncthreads();
@@ -601,20 +605,27 @@ k_label(const SweepArgs a)
     // ---- union, in log2(TH) waves: wave j joins blocks of 2^(j-1) rows pairwise, so every wave
     //      links roots of forests that are already flat and the trees stay shallow.  The bonds of a
     //      wave are dealt out evenly to ALL threads from the wave's list.
+    auto unite_at = [&](uint32_t site) {
+        const uint32_t rt = site / TW, col = site % TW, ww = col >> 5, c = col & 31u;
+        const uint32_t m = (2u << c) - 1u;                                         // bits <= c
+        const uint32_t mt = Ss[rt][ww] & m, mb = Ss[rt + 1][ww] & m;
+        const uint32_t bt = site - c;
+        const uint32_t at = mt ? bt + 31 - __clz(mt) : LLs[rt][ww];
+        const uint32_t ab = mb ? bt + TW + 31 - __clz(mb) : LLs[rt + 1][ww];
+        sunion_v(parent, at, ab);
+    };
 #pragma unroll 1
     for (int j = 1; (1 << j) <= TH; ++j) {
-        const uint32_t n = wcnt[j];
-        const uint16_t *lst = wlist + (TW * TH - TW * (TH >> (j - 1)));
+        const uint32_t n = min(wcnt[j], (uint32_t)(LCAP >> j));
+        const uint16_t *lst = wlist + (LCAP - (LCAP >> (j - 1)));
         const uint32_t per = (n + NT - 1) / NT, i1 = min(n, (tid + 1) * per);
-        for (uint32_t i = tid * per; i < i1; ++i) {           // contiguous share: neighbouring bonds mostly join the same runs
-            const uint32_t site = lst[i];
-            const uint32_t rt = site / TW, col = site % TW, ww = col >> 5, c = col & 31u;
-            const uint32_t m = (2u << c) - 1u;                                     // bits <= c
-            const uint32_t mt = Ss[rt][ww] & m, mb = Ss[rt + 1][ww] & m;
-            const uint32_t bt = site - c;
-            const uint32_t at = mt ? bt + 31 - __clz(mt) : LLs[rt][ww];
-            const uint32_t ab = mb ? bt + TW + 31 - __clz(mb) : LLs[rt + 1][ww];
-            sunion_v(parent, at, ab);
+        for (uint32_t i = tid * per; i < i1; ++i) unite_at(lst[i]);   // contiguous share: neighbouring bonds mostly join the same runs
+        if (myj == j) {
+            while (need) {                                            // overflow of the list (dense y bonds): this thread's own
+                const int c = __ffs(need) - 1;
+                need &= need - 1;
+                unite_at(base + c);
+            }
         }
         __syncthreads();
     }
