@@ -218,6 +218,7 @@ def main():
     ap.add_argument("--labels64", action="store_true", help="hold labels as 64-bit words")
     ap.add_argument("--fourier", action="store_true",
                     help="also reduce the structure-factor sums of every sweep (xi_2nd; XY_FLAG_FOURIER)")
+    ap.add_argument("--beta", type=float, default=None, help="override the workload's beta (sensitivity runs)")
     ap.add_argument("--e2e-steps", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -241,6 +242,8 @@ def main():
     barrier, max_over_ranks = grp.barrier, grp.max_over_ranks
 
     cfg_idx, L, init, seed, beta, therm = WORKLOADS[args.workload]
+    if args.beta is not None:
+        beta = args.beta
     N = L * L
     flags = (xy.FLAG_LABELS64 if args.labels64 else 0) | (xy.FLAG_FOURIER if args.fourier else 0)
     label_bytes = 8 if args.labels64 else 4
