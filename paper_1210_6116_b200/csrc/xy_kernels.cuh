@@ -717,11 +717,11 @@ k_merge(const SweepArgs a)
                 lb = gload(labels + (size_t)y2 * L + x2);
             }
         }
-        // neighbouring edge bonds mostly join the same two tile-local components: the lane to the
-        // left already does that union (it never skips unless ITS left neighbour does the same one)
-        const LabelT pa = __shfl_up_sync(0xffffffffu, la, 1), pb = __shfl_up_sync(0xffffffffu, lb, 1);
-        const bool pact = __shfl_up_sync(0xffffffffu, (int)active, 1) != 0;
-        const bool dup = (threadIdx.x & 31) != 0 && pact && pa == la && pb == lb;
+        // the edge bonds of a tile mostly join the same few pairs of tile-local components: of all
+        // lanes of the warp with the same (la, lb) only the lowest does the union
+        const uint32_t act = __ballot_sync(0xffffffffu, active);
+        const uint32_t same = __match_any_sync(0xffffffffu, la) & __match_any_sync(0xffffffffu, lb) & act;
+        const bool dup = (same & ((1u << (threadIdx.x & 31)) - 1u)) != 0;
         if (active && !dup) gunion<LabelT>(labels, la, lb);
     }
 }
