@@ -127,7 +127,8 @@ int xy_create_ex(xy_state **out, uint32_t L, uint64_t seed, int init, uint32_t f
 
 /* ---- parity / checkpoint extensions (host buffers; each synchronises the state's stream) ----- */
 
-int xy_get_angles(xy_state *s, float *host, size_t n);          /* n must equal L*L */
+/* the getters below copy the first n sites (row-major), 1 <= n <= L*L */
+int xy_get_angles(xy_state *s, float *host, size_t n);
 int xy_set_angles(xy_state *s, const float *host, size_t n);    /* values must lie in [0, 6.2831855] */
 /* canonical labels of the most recent sweep, label = minimum site index of the cluster, widened
  * to int64 for every L; XY_ERR_STATE before the first sweep. */

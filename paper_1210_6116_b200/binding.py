@@ -188,9 +188,11 @@ class XYState:
             pass
 
     # -- extensions -------------------------------------------------------------------------
-    def get_angles(self, out=None):
-        out = np.empty(self.N, np.float32) if out is None else out
-        _check(_lib.xy_get_angles(self._h, _host_ptr(out), self.N))
+    def get_angles(self, out=None, n=None):
+        """the first n sites (default: all)"""
+        n = self.N if n is None else int(n)
+        out = np.empty(n, np.float32) if out is None else out
+        _check(_lib.xy_get_angles(self._h, _host_ptr(out), n))
         return out
 
     def set_angles(self, theta):
@@ -198,14 +200,16 @@ class XYState:
             theta = np.ascontiguousarray(theta, np.float32)
         _check(_lib.xy_set_angles(self._h, _host_ptr(theta), self.N))
 
-    def get_labels(self):
-        out = np.empty(self.N, np.int64)
-        _check(_lib.xy_get_labels(self._h, out.ctypes.data, self.N))
+    def get_labels(self, n=None):
+        n = self.N if n is None else int(n)
+        out = np.empty(n, np.int64)
+        _check(_lib.xy_get_labels(self._h, out.ctypes.data, n))
         return out
 
-    def get_bonds(self):
-        out = np.empty(self.N, np.uint8)
-        _check(_lib.xy_get_bonds(self._h, out.ctypes.data, self.N))
+    def get_bonds(self, n=None):
+        n = self.N if n is None else int(n)
+        out = np.empty(n, np.uint8)
+        _check(_lib.xy_get_bonds(self._h, out.ctypes.data, n))
         return out
 
     def measure_fourier(self):

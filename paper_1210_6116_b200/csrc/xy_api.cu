@@ -642,7 +642,7 @@ int xy_pcc_run(xy_state *s, double beta0, double dbeta0, const xy_pcc_schedule *
 int xy_get_angles(xy_state *s, float *host, size_t n)
 {
     if (!s || !host) return fail(XY_ERR_ARG, "NULL argument");
-    if (n != s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
+    if (n == 0 || n > s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
     DeviceGuard g(s->device);
     CUDA_TRY(cudaMemcpyAsync(host, s->theta(), n * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
     CUDA_TRY(cudaStreamSynchronize(s->stream));
@@ -778,7 +778,7 @@ int xy_get_fallback_count(xy_state *s, uint64_t *count)
 int xy_get_labels(xy_state *s, int64_t *host, size_t n)
 {
     if (!s || !host) return fail(XY_ERR_ARG, "NULL argument");
-    if (n != s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
+    if (n == 0 || n > s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
     if (!s->have_sweep) return fail(XY_ERR_STATE, "no sweep has produced labels yet");
     DeviceGuard g(s->device);
     if (int rc = ensure_stage(s)) return rc;
@@ -789,8 +789,8 @@ int xy_get_labels(xy_state *s, int64_t *host, size_t n)
         s->labels_flat = true;
     }
     const uint64_t chunk = kStageBytes / sizeof(int64_t);
-    for (uint64_t first = 0; first < s->N; first += chunk) {
-        const uint64_t m = s->N - first < chunk ? s->N - first : chunk;
+    for (uint64_t first = 0; first < n; first += chunk) {
+        const uint64_t m = n - first < chunk ? n - first : chunk;
         if (s->l64()) k_labels_to_i64<uint64_t><<<148 * 4, 256, 0, s->stream>>>(static_cast<const uint64_t *>(s->labels()), static_cast<int64_t *>(s->stage), first, m);
         else k_labels_to_i64<uint32_t><<<148 * 4, 256, 0, s->stream>>>(static_cast<const uint32_t *>(s->labels()), static_cast<int64_t *>(s->stage), first, m);
         CUDA_TRY(cudaMemcpyAsync(host + first, s->stage, m * sizeof(int64_t), cudaMemcpyDeviceToHost, s->stream));
@@ -802,13 +802,13 @@ int xy_get_labels(xy_state *s, int64_t *host, size_t n)
 int xy_get_bonds(xy_state *s, uint8_t *host, size_t n)
 {
     if (!s || !host) return fail(XY_ERR_ARG, "NULL argument");
-    if (n != s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
+    if (n == 0 || n > s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
     if (!s->have_sweep) return fail(XY_ERR_STATE, "no sweep has produced bonds yet");
     DeviceGuard g(s->device);
     if (int rc = ensure_stage(s)) return rc;
     const uint64_t chunk = kStageBytes;
-    for (uint64_t first = 0; first < s->N; first += chunk) {
-        const uint64_t m = s->N - first < chunk ? s->N - first : chunk;
+    for (uint64_t first = 0; first < n; first += chunk) {
+        const uint64_t m = n - first < chunk ? n - first : chunk;
         k_bonds_unpack<<<148 * 4, 256, 0, s->stream>>>(s->bonds(), static_cast<uint8_t *>(s->stage), first, m);
         CUDA_TRY(cudaMemcpyAsync(host + first, s->stage, m, cudaMemcpyDeviceToHost, s->stream));
         CUDA_TRY(cudaStreamSynchronize(s->stream));
