@@ -1,0 +1,56 @@
+"""The paper's PCC protocol on the GPU (beta*Upsilon against 0.636508 over windows of
+1000 MCS, dbeta = 5e-4, 60 000 MCS discarded), shortened to 3e5 measured sweeps, against Table I
+(PAPER.md:80-84): beta_KT(L), <m^2>_L and xi_2nd(L)/L for L = 64 and 128.  Statistical pins: the paper's
+error bars are for 4e6 MCS; ours are ~3.5 times wider.  Observed on the first run: beta_KT 1.09231 / 1.09808
+(paper 1.09167(25) / 1.09788(32)), <m^2> 0.34985 / 0.29574 (0.34924(29) / 0.29695(36)), xi_2nd/L 0.7484 /
+0.7474 (0.7464(11) / 0.7466(15)); the tolerances are about 3 of our standard errors."""
+import numpy as np
+import pytest
+
+from golden_io import constants, table1
+from oracle import xy_oracle as xo
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def xy():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1210_6116_b200 as m
+    return m
+
+
+@pytest.mark.parametrize("L,seed", [(64, 21), (128, 22)])
+def test_paper_protocol_table1(xy, L, seed):
+    row = table1()[L]
+    c = constants()
+    target, dbeta = c["betaY_critical"], c["pcc_dbeta"]
+    assert (int(c["pcc_window_mcs"]), int(c["pcc_discard_mcs"])) == (1000, 60000)
+    discard, windows = 60000, 300
+    sched = xy.PccSchedule(n_sweeps=discard + 1000 * windows, discard=discard, window=1000, dirs=1,
+                           dbeta0=dbeta, halve_every=0, dbeta_min=dbeta, target=target)
+    st = xy.XYState(L, seed, xy.INIT_HOT, flags=xy.FLAG_FOURIER)
+    out = st.pcc_run(1.10, sched)
+    tb = out["trace_beta"]
+    assert out["n_decisions"] == windows and tb.size == windows
+    beta_kt = tb.mean()
+    # beta walks in steps of 5e-4 around the crossing; the mean over 300 windows is good to ~1e-3
+    assert abs(beta_kt - row["beta"]) < 2.5e-3, (beta_kt, row["beta"])
+    # <m^2> and xi_2nd / L over the records the device ring still holds (the last 16383 sweeps of the walk)
+    T = st.get_sweep()
+    cap = st.series_capacity()
+    n = min(cap - 1, 16000)
+    obs = st.get_series(T - n + 1, n)
+    fou = st.get_fourier_series(T - n + 1, n)
+    N = L * L
+    m2 = ((obs["Mx"] ** 2 + obs["My"] ** 2) / N ** 2).mean()
+    assert abs(m2 - row["m2"]) < 0.005, (m2, row["m2"])
+    chi0 = N * m2
+    chik = 0.5 * ((fou["Fx"] ** 2).sum(axis=1).mean() + (fou["Fy"] ** 2).sum(axis=1).mean()) / N
+    xi_over_L = xo.xi2nd(chi0, chik, L) / L
+    assert abs(xi_over_L - row["xi"]) < 0.012, (xi_over_L, row["xi"])
+    print(f"L={L}: beta_KT {beta_kt:.5f} (paper {row['beta']}), m2 {m2:.5f} (paper {row['m2']}), "
+          f"xi/L {xi_over_L:.4f} (paper {row['xi']})")
+    st.destroy()
