@@ -1,5 +1,5 @@
 // xy_device.cuh -- device-side building blocks of the XY Swendsen-Wang sweep for sm_100a:
-// Philox4x32-10, fp64 sincos on [0, 2pi], the filtered bond decision, union-find helpers,
+// Philox4x32-10, the filtered bond decision, the reflection, global union-find helpers,
 // warp / block reductions.  Product code: shares nothing with oracle/.
 #pragma once
 #include <cuda_runtime.h>
@@ -59,44 +59,6 @@ __device__ __forceinline__ U4 philox4x32_10_rk(uint32_t c0, uint32_t c1, uint32_
 __host__ __device__ __forceinline__ U4 rng(uint32_t seed_lo, uint32_t seed_hi, uint64_t idx, uint32_t t, uint32_t tag)
 {
     return philox4x32_10((uint32_t)idx, (uint32_t)(idx >> 32), t, tag, seed_lo, seed_hi);
-}
-
-// ---------------------------------------------------------------------------------------------
-// sin and cos of an fp32 angle in [0, 2pi] (any |theta| < ~100 is fine), evaluated in fp64 with
-// |error| < 5e-13: Cody-Waite reduction by pi/2 in two pieces, Taylor polynomials on |r| <= pi/4
-// (sin through r^13: remainder (pi/4)^15/15! = 2e-14; cos through r^12: (pi/4)^14/14! = 4e-13).
-// This feeds the observables (tolerance 1e-9 per term) and the bond FILTER; bond decisions the
-// filter cannot settle are re-evaluated with libdevice cos/expm1 (bond_exact below).
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ void sincos_poly(float theta, double &s, double &c)
-{
-    const double t = (double)theta;
-    const double kd = __fma_rn(t, 0.6366197723675814, 6755399441055744.0);   // t * 2/pi, rounded to integer
-    const int q = __double2loint(kd);
-    const double k = kd - 6755399441055744.0;
-    double r = __fma_rn(-k, 1.5707963267948966, t);          // pi/2 high part
-    r = __fma_rn(-k, 6.123233995736766e-17, r);              // pi/2 low part
-    const double z = r * r;
-    double ps = -7.6471637318198164759e-13;                  // -1/15!
-    ps = __fma_rn(ps, z, 1.6059043836821614599e-10);         //  1/13!
-    ps = __fma_rn(ps, z, -2.5052108385441718775e-8);         // -1/11!
-    ps = __fma_rn(ps, z, 2.7557319223985890653e-6);          //  1/9!
-    ps = __fma_rn(ps, z, -1.9841269841269841270e-4);         // -1/7!
-    ps = __fma_rn(ps, z, 8.3333333333333333333e-3);          //  1/5!
-    ps = __fma_rn(ps, z, -1.6666666666666666667e-1);         // -1/3!
-    const double sr = __fma_rn(ps * z, r, r);
-    double pc = 2.0876756987868098979e-9;                    //  1/12!
-    pc = __fma_rn(pc, z, -2.7557319223985890653e-7);         // -1/10!
-    pc = __fma_rn(pc, z, 2.4801587301587301587e-5);          //  1/8!
-    pc = __fma_rn(pc, z, -1.3888888888888888889e-3);         // -1/6!
-    pc = __fma_rn(pc, z, 4.1666666666666666667e-2);          //  1/4!
-    pc = __fma_rn(pc, z, -0.5);
-    const double cr = __fma_rn(pc, z, 1.0);
-    // quadrant: q&1 swaps, q&2 negates sin, (q+1)&2 negates cos
-    const double a = (q & 1) ? cr : sr;
-    const double b = (q & 1) ? sr : cr;
-    s = (q & 2) ? -a : a;
-    c = ((q + 1) & 2) ? -b : b;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -171,37 +133,9 @@ __device__ __forceinline__ float reflect(float theta, double A)
 }
 
 // ---------------------------------------------------------------------------------------------
-// Union-find in shared memory (tile-local) and global memory (boundary merge).  Links always go
-// from the larger to the smaller index, so the root of a component is its minimum index.
+// Union-find in global memory (boundary merge; the tile-local one lives with k_label).  Links always
+// go from the larger to the smaller index, so the root of a component is its minimum index.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t sfind(const volatile uint32_t *p, uint32_t a)
-{
-    uint32_t r = p[a];
-    while (r != a) { a = r; r = p[a]; }
-    return a;
-}
-
-// Both chains advance in lock step (two independent loads per round); a node that already is a
-// root re-reads itself.  Links go from the larger root to the smaller one.
-__device__ __forceinline__ void sunion(uint32_t *p, uint32_t a, uint32_t b)
-{
-    const volatile uint32_t *vp = p;
-    for (;;) {
-        if (a == b) return;
-        const uint32_t pa = vp[a], pb = vp[b];
-        if (pa == a && pb == b) {
-            const uint32_t hi = a > b ? a : b, lo = a > b ? b : a;
-            const uint32_t old = atomicMin(&p[hi], lo);
-            if (old == hi) return;
-            a = old;                                             // hi was re-linked meanwhile: carry on with its parent
-            b = lo;
-        } else {
-            a = pa;
-            b = pb;
-        }
-    }
-}
-
 template <typename T> struct AtomT;
 template <> struct AtomT<uint32_t> { using type = unsigned int; };
 template <> struct AtomT<uint64_t> { using type = unsigned long long; };

@@ -4,12 +4,13 @@
 //             by row: theta -> fp64 (cos, sin, sigma) per site in registers (table + short Taylor
 //             rotation) -> observables, Philox bond draws, filtered bond decisions -> packed bond
 //             bits (0.25 B/site).  theta is read once (+ halo); no block barrier in the loop.
-//   k_label   (S3): one CTA per TW x TH tile, integer only: run starts by ballot/clz over the
-//             x-bond bits, union-find over the runs in shared memory -> provisional label (global
-//             index of the tile-local root), written once.
-//   k_merge        (S4): one thread per tile-edge bond; atomicMin union-find on the label array.
-//   k_flip         (S5+S6): chase each site's label to the cluster's root (minimum site index),
-//                  draw the root's coin with Philox, reflect, write theta back.
+//   k_label   (S3): one CTA per TW x TH tile, integer only, bit-parallel: a thread holds the x / y
+//             bond bits of 32 sites in two registers; union-find over RUNS of x bonds in shared
+//             memory, united in log2(TH) waves -> provisional label (global index of the
+//             tile-local root) and one root bit per site, written once.
+//   k_merge   (S4): one thread per tile-edge bond; atomicMin union-find on the label array.
+//   k_flip    (S5+S6): coins of a tile's labels from one Philox call per tile row; tile roots
+//             that k_merge linked elsewhere chase their root; reflect, write theta back.
 //   finalize       (S8): the last CTA of k_bonds reduces the per-CTA partial sums in a fixed
 //                  order, writes the per-sweep record and advances the PCC controller.
 //
@@ -176,7 +177,7 @@ k_bonds(const SweepArgs a)
 
     __shared__ double2 tab[kTabN + 1];
     __shared__ double h_c[NW][RS], h_s[NW][RS];
-    __shared__ float h_t[NW][RS], h_g[NW][RS];
+    __shared__ float h_g[NW][RS];
     __shared__ double red[NW][NS];
     __shared__ double2 h_ky[kFourier ? NW : 1][RS];      // (cos, sin)(2 pi y / L) of the strip's rows
     __shared__ unsigned long long redc[NW][2];
@@ -215,7 +216,6 @@ k_bonds(const SweepArgs a)
             const float th = __ldg(a.theta + (size_t)(y0 + lane) * L + xh);
             double s, c;
             sincos_tab(th, tab, s, c);
-            h_t[warp][lane] = th;
             h_c[warp][lane] = c;
             h_s[warp][lane] = s;
             h_g[warp][lane] = __double2float_rn(__fma_rn(c, cphi, s * sphi));
