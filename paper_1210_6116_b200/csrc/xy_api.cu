@@ -77,19 +77,21 @@ struct Kernels {
     int tw, th, rs;
 };
 
-constexpr int kRS = 32;          // rows per warp strip in k_bonds
+// rows per warp strip in k_bonds: 32 (1/32 halo recompute) on large lattices; 8 where 32-row strips would
+// leave warps without work or with one long serial strip (L <= 4096: fewer than 2 strips per resident warp)
+constexpr int kRSLarge = 32, kRSSmall = 8;
 constexpr int kBondsWarps = 4;   // warps per CTA in k_bonds
 
-template <int VEC, int R, int NW, typename LabelT>
+template <int VEC, int R, int NW, int RS, typename LabelT>
 struct KS {
     static void bonds(const SweepArgs &a, bool obs_only, bool fourier, int grid, cudaStream_t st)
     {
         if (fourier) {
-            if (obs_only) k_bonds<VEC, kRS, false, true><<<grid, kBondsWarps * 32, 0, st>>>(a);
-            else k_bonds<VEC, kRS, true, true><<<grid, kBondsWarps * 32, 0, st>>>(a);
+            if (obs_only) k_bonds<VEC, RS, false, true><<<grid, kBondsWarps * 32, 0, st>>>(a);
+            else k_bonds<VEC, RS, true, true><<<grid, kBondsWarps * 32, 0, st>>>(a);
         } else {
-            if (obs_only) k_bonds<VEC, kRS, false, false><<<grid, kBondsWarps * 32, 0, st>>>(a);
-            else k_bonds<VEC, kRS, true, false><<<grid, kBondsWarps * 32, 0, st>>>(a);
+            if (obs_only) k_bonds<VEC, RS, false, false><<<grid, kBondsWarps * 32, 0, st>>>(a);
+            else k_bonds<VEC, RS, true, false><<<grid, kBondsWarps * 32, 0, st>>>(a);
         }
     }
     static void label(const SweepArgs &a, cudaStream_t st)
@@ -117,18 +119,18 @@ struct KS {
     static int occupancy(bool fourier, int *bonds_sweep, int *bonds_obs, int *fl)
     {
         cudaError_t e;
-        if (fourier) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_sweep, k_bonds<VEC, kRS, true, true>, kBondsWarps * 32, 0);
-        else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_sweep, k_bonds<VEC, kRS, true, false>, kBondsWarps * 32, 0);
+        if (fourier) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_sweep, k_bonds<VEC, RS, true, true>, kBondsWarps * 32, 0);
+        else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_sweep, k_bonds<VEC, RS, true, false>, kBondsWarps * 32, 0);
         if (e != cudaSuccess) return (int)e;
-        if (fourier) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_obs, k_bonds<VEC, kRS, false, true>, kBondsWarps * 32, 0);
-        else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_obs, k_bonds<VEC, kRS, false, false>, kBondsWarps * 32, 0);
+        if (fourier) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_obs, k_bonds<VEC, RS, false, true>, kBondsWarps * 32, 0);
+        else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_obs, k_bonds<VEC, RS, false, false>, kBondsWarps * 32, 0);
         if (e != cudaSuccess) return (int)e;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(fl, k_flip<VEC, R * NW, LabelT>, VEC * R * NW, 0);
         return (int)e;
     }
     static Kernels get()
     {
-        return Kernels{&bonds, &label, &merge, &flip, &occupancy, 32 * VEC, R * NW, kRS};
+        return Kernels{&bonds, &label, &merge, &flip, &occupancy, 32 * VEC, R * NW, RS};
     }
 };
 
@@ -136,8 +138,13 @@ constexpr int kR = 4, kNW = 8;   // label / flip tiles: TH = kR * kNW = 32 rows;
 
 Kernels pick_kernels(uint32_t L, bool l64)
 {
-    if (L % 128 == 0) return l64 ? KS<4, kR, kNW, uint64_t>::get() : KS<4, kR, kNW, uint32_t>::get();
-    return l64 ? KS<2, kR, kNW, uint64_t>::get() : KS<2, kR, kNW, uint32_t>::get();
+    const bool small = L <= 4096;
+    if (L % 128 == 0) {
+        if (small) return l64 ? KS<4, kR, kNW, kRSSmall, uint64_t>::get() : KS<4, kR, kNW, kRSSmall, uint32_t>::get();
+        return l64 ? KS<4, kR, kNW, kRSLarge, uint64_t>::get() : KS<4, kR, kNW, kRSLarge, uint32_t>::get();
+    }
+    if (small) return l64 ? KS<2, kR, kNW, kRSSmall, uint64_t>::get() : KS<2, kR, kNW, kRSSmall, uint32_t>::get();
+    return l64 ? KS<2, kR, kNW, kRSLarge, uint64_t>::get() : KS<2, kR, kNW, kRSLarge, uint32_t>::get();
 }
 
 __global__ void k_debug_curand_philox(const uint32_t *ctr, const uint32_t *key, uint32_t *out, size_t n)
