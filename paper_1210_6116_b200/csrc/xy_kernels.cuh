@@ -745,7 +745,8 @@ k_flip(const SweepArgs a)
     constexpr int TW = 32 * WPR, NT = WPR * TH;
     constexpr int Q = TW / 4, RPP = NT / Q, NP = TH / RPP;
     __shared__ uint32_t cbits[TH * WPR];             // coin of the tile root at tile-local index loc: bit loc
-    __shared__ uint32_t queue[2 * (TW + TH)];        // merged tile roots: each owns a component that touches the tile edge, so at most one per edge site
+    __shared__ uint16_t queue[2 * (TW + TH)];        // merged tile roots: each owns a component that touches the tile edge, so at most one per edge site
+    __shared__ float4 th_s[NP * NT];                 // the tile's angles, staged by cp.async while the label phases run
     __shared__ uint32_t nqueue;
     __shared__ unsigned long long sc[NT / 32];
 
@@ -757,6 +758,16 @@ k_flip(const SweepArgs a)
     const uint32_t x0 = tx * TW, y0 = ty * TH;
     const int q = tid % Q, rq = tid / Q;
     const LabelT gbase = (LabelT)y0 * L + x0;
+
+    // theta of my 4 x NP sites -> shared memory, asynchronously (no registers held): its DRAM latency
+    // hides behind the label phases; each thread later reads back exactly what it copied
+#pragma unroll
+    for (int k = 0; k < NP; ++k) {
+        const size_t i = (size_t)(y0 + k * RPP + rq) * L + x0 + 4 * q;
+        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&th_s[k * NT + tid]);
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(a.theta + i) : "memory");
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
 
     if (tid == 0) nqueue = 0;
     if (tid < TH) {
@@ -804,7 +815,7 @@ k_flip(const SweepArgs a)
     while (merged) {
         const int b = __ffs(merged) - 1;
         merged &= merged - 1;
-        queue[atomicAdd(&nqueue, 1u)] = ((b >> 2) * RPP + rq) * TW + 4 * q + (b & 3);
+        queue[atomicAdd(&nqueue, 1u)] = (uint16_t)(((b >> 2) * RPP + rq) * TW + 4 * q + (b & 3));
     }
     __syncthreads();
     {
@@ -825,13 +836,14 @@ k_flip(const SweepArgs a)
     __syncthreads();
 
     // ---- every site takes the coin of its tile root; reflect ----
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
     const uint32_t Lm = L - TW;
 #pragma unroll
     for (int k = 0; k < NP; ++k) {
         const int row = k * RPP + rq;
         const uint32_t loc0 = row * TW + 4 * q;
         const size_t i = (size_t)(y0 + row) * L + x0 + 4 * q;
-        const float4 t4 = *reinterpret_cast<const float4 *>(a.theta + i);
+        const float4 t4 = th_s[k * NT + tid];
         const float th[4] = {t4.x, t4.y, t4.z, t4.w};
         LabelT lab[4];
         load_labels(i, lab);
