@@ -98,10 +98,11 @@ def test_cfg4_full_size_sweep(xy):
     assert rec.sweep == t + 1 and rec.beta == beta
 
 
-def test_cfg5_prefix_rows(xy):
+@pytest.mark.parametrize("flags", [0, 1])              # 1: labels held as 64-bit words (north_star: int64 from L = 65536)
+def test_cfg5_prefix_rows(xy, flags):
     L, seed, beta, R = 65536, 17, 1.11996, 96
     n = R * L
-    st = xy.XYState(L, seed, xy.INIT_HOT)
+    st = xy.XYState(L, seed, xy.INIT_HOT, flags=flags)
     st.sw_sweeps(beta, 1)
     t = st.get_sweep()
     th0 = st.get_angles(n=n)
