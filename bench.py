@@ -291,10 +291,13 @@ def main():
     sweep_bytes = sum(model.values())
     sweep_gbs = sweep_bytes * N * K / (ms * 1e-3) / 1e9
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")      # workload,kernel,dram_bytes_per_launch (from ncu)
     if os.path.exists(tpath):
         try:
-            traffic = json.load(open(tpath)).get(args.workload, {}).get(dom)
+            for row in open(tpath).read().split()[1:]:
+                w, kname, nbytes = row.split(",")
+                if w == args.workload and kname == dom:
+                    traffic = int(nbytes)
         except Exception:
             traffic = None
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["achieved_gbs"], "peak": peak,
