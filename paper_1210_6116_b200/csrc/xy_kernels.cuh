@@ -605,14 +605,11 @@ k_label(const SweepArgs a)
     // ---- union, in log2(TH) waves: wave j joins blocks of 2^(j-1) rows pairwise, so every wave
     //      links roots of forests that are already flat and the trees stay shallow.  The bonds of a
     //      wave are dealt out evenly to ALL threads from the wave's list.
+    // parent[site] is the site's run start, or (for a run start that was linked already) an ancestor of
+    // it: either way a node of the right component to start the finds from
     auto unite_at = [&](uint32_t site) {
-        const uint32_t rt = site / TW, col = site % TW, ww = col >> 5, c = col & 31u;
-        const uint32_t m = (2u << c) - 1u;                                         // bits <= c
-        const uint32_t mt = Ss[rt][ww] & m, mb = Ss[rt + 1][ww] & m;
-        const uint32_t bt = site - c;
-        const uint32_t at = mt ? bt + 31 - __clz(mt) : LLs[rt][ww];
-        const uint32_t ab = mb ? bt + TW + 31 - __clz(mb) : LLs[rt + 1][ww];
-        sunion_v(parent, at, ab);
+        const volatile uint32_t *vp = parent;
+        sunion_v(parent, vp[site], vp[site + TW]);
     };
 #pragma unroll 1
     for (int j = 1; (1 << j) <= TH; ++j) {
