@@ -474,38 +474,37 @@ __device__ __forceinline__ uint32_t nib_lo16(uint32_t v)      // low nibbles of 
     return (t | (t >> 8)) & 0xFFFFu;
 }
 
-__device__ __forceinline__ uint32_t sfind_v(const volatile uint32_t *p, uint32_t a)
+// The tile-local union-find stores parents as BYTE offsets into parent[] (index * 4): a hop is one
+// shared load at [value + base] with no address arithmetic.  Order and equality are those of the indices.
+__device__ __forceinline__ uint32_t pload(const unsigned char *pb, uint32_t off)
 {
-    uint32_t r = p[a];
-    while (r != a) { a = r; r = p[a]; }
-    return a;
+    return *reinterpret_cast<const volatile uint32_t *>(pb + off);
 }
 
 // find with path halving: every node on the way is re-pointed to its grandparent.  Racing writers
 // only ever replace a parent by an ancestor, so concurrent finds and min-links stay correct.
-__device__ __forceinline__ uint32_t sfind_h(volatile uint32_t *p, uint32_t a)
+__device__ __forceinline__ uint32_t sfind_h(unsigned char *pb, uint32_t a)
 {
-    uint32_t r = p[a];
+    uint32_t r = pload(pb, a);
     while (r != a) {
-        const uint32_t g = p[r];
+        const uint32_t g = pload(pb, r);
         if (g == r) return r;
-        p[a] = g;
+        *reinterpret_cast<volatile uint32_t *>(pb + a) = g;
         a = g;
-        r = p[a];
+        r = pload(pb, a);
     }
     return a;
 }
 
-// min-link union of the components of a and b (any nodes)
-__device__ __forceinline__ void sunion_v(uint32_t *p, uint32_t a, uint32_t b)
+// min-link union of the components of a and b (any nodes; byte offsets)
+__device__ __forceinline__ void sunion_v(unsigned char *pb, uint32_t a, uint32_t b)
 {
-    volatile uint32_t *vp = p;
     for (;;) {
-        a = sfind_h(vp, a);
-        b = sfind_h(vp, b);
+        a = sfind_h(pb, a);
+        b = sfind_h(pb, b);
         if (a == b) return;
         const uint32_t hi = a > b ? a : b, lo = a > b ? b : a;
-        const uint32_t old = atomicMin(&p[hi], lo);
+        const uint32_t old = atomicMin(reinterpret_cast<uint32_t *>(pb + hi), lo);
         if (old == hi) return;
         a = old;                                   // hi was linked meanwhile: go on from its new parent
         b = lo;
@@ -573,10 +572,10 @@ k_label(const SweepArgs a)
         const uint32_t wbase = row * TW + 32 * wq;
         const uint32_t m = Sq & ((2u << o) - 1u);
         uint4 st;
-        st.x = m ? wbase + 31 - __clz(m) : LLs[row][wq];
-        st.y = ((Sq >> (o + 1)) & 1u) ? wbase + o + 1 : st.x;
-        st.z = ((Sq >> (o + 2)) & 1u) ? wbase + o + 2 : st.y;
-        st.w = ((Sq >> (o + 3)) & 1u) ? wbase + o + 3 : st.z;
+        st.x = (m ? wbase + 31 - __clz(m) : LLs[row][wq]) * 4u;              // byte offsets (see pload)
+        st.y = ((Sq >> (o + 1)) & 1u) ? (wbase + o + 1) * 4u : st.x;
+        st.z = ((Sq >> (o + 2)) & 1u) ? (wbase + o + 2) * 4u : st.y;
+        st.w = ((Sq >> (o + 3)) & 1u) ? (wbase + o + 3) * 4u : st.z;
         *reinterpret_cast<uint4 *>(&parent[wbase + o]) = st;
     }
 
@@ -607,9 +606,9 @@ k_label(const SweepArgs a)
     //      wave are dealt out evenly to ALL threads from the wave's list.
     // parent[site] is the site's run start, or (for a run start that was linked already) an ancestor of
     // it: either way a node of the right component to start the finds from
+    unsigned char *pb = reinterpret_cast<unsigned char *>(parent);
     auto unite_at = [&](uint32_t site) {
-        const volatile uint32_t *vp = parent;
-        sunion_v(parent, vp[site], vp[site + TW]);
+        sunion_v(pb, pload(pb, site * 4u), pload(pb, (site + TW) * 4u));
     };
 #pragma unroll 1
     for (int j = 1; (1 << j) <= TH; ++j) {
@@ -636,7 +635,7 @@ k_label(const SweepArgs a)
             const uint32_t i0 = (k * RPP + rq) * TW + 4 * q;
             const uint4 p1 = *reinterpret_cast<const uint4 *>(&parent[i0]);
             uint4 p2;
-            p2.x = parent[p1.x]; p2.y = parent[p1.y]; p2.z = parent[p1.z]; p2.w = parent[p1.w];
+            p2.x = pload(pb, p1.x); p2.y = pload(pb, p1.y); p2.z = pload(pb, p1.z); p2.w = pload(pb, p1.w);
             *reinterpret_cast<uint4 *>(&parent[i0]) = p2;
         }
     }
@@ -652,18 +651,19 @@ k_label(const SweepArgs a)
         {
             uint32_t up[4];
 #pragma unroll
-            for (int v = 0; v < 4; ++v) up[v] = parent[root[v]];
+            for (int v = 0; v < 4; ++v) up[v] = pload(pb, root[v]);
             while (up[0] != root[0] || up[1] != root[1] || up[2] != root[2] || up[3] != root[3]) {   // rare: a longer chain
 #pragma unroll
-                for (int v = 0; v < 4; ++v) { root[v] = up[v]; up[v] = parent[root[v]]; }
+                for (int v = 0; v < 4; ++v) { root[v] = up[v]; up[v] = pload(pb, root[v]); }
             }
         }
         LabelT out[4];
         uint32_t nib = 0;
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
-            out[v] = gbase + (LabelT)(root[v] / TW) * L + (root[v] % TW);
-            nib |= (root[v] == i0 + v) ? (1u << v) : 0u;
+            const uint32_t rl = root[v] >> 2;                            // byte offset -> tile-local index
+            out[v] = gbase + (LabelT)(rl / TW) * L + (rl % TW);
+            nib |= (rl == i0 + v) ? (1u << v) : 0u;
         }
         const size_t gi = (size_t)(y0 + row) * L + x0 + 4 * q;
         LabelT *dst = labels + gi;
