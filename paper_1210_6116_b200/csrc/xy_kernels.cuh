@@ -465,7 +465,7 @@ k_bonds(const SweepArgs a)
 // Bonds that leave the tile are left to k_merge.
 // ---------------------------------------------------------------------------------------------
 template <int WPR, int TH>
-constexpr size_t k_label_smem_bytes() { return (size_t)(32 * WPR) * TH * 4 + (size_t)TH * WPR * 12 + (size_t)(32 * WPR) * TH + 32; }
+constexpr size_t k_label_smem_bytes() { return (size_t)(32 * WPR) * TH * 2 + (size_t)TH * WPR * 12 + (size_t)(32 * WPR) * TH + 32; }
 
 __device__ __forceinline__ uint32_t nib_lo16(uint32_t v)      // low nibbles of 4 bytes -> 16 bits
 {
@@ -474,11 +474,28 @@ __device__ __forceinline__ uint32_t nib_lo16(uint32_t v)      // low nibbles of 
     return (t | (t >> 8)) & 0xFFFFu;
 }
 
-// The tile-local union-find stores parents as BYTE offsets into parent[] (index * 4): a hop is one
-// shared load at [value + base] with no address arithmetic.  Order and equality are those of the indices.
+// The tile-local union-find stores parents as 16-bit BYTE offsets into parent[] (index * 2; a tile has
+// at most 2^15 sites): a hop is one shared load at [value + base] with no address arithmetic, and the
+// array is half the size of 32-bit indices (shared memory bounds the CTAs per SM of k_label).  Order
+// and equality are those of the indices.
 __device__ __forceinline__ uint32_t pload(const unsigned char *pb, uint32_t off)
 {
-    return *reinterpret_cast<const volatile uint32_t *>(pb + off);
+    return *reinterpret_cast<const volatile uint16_t *>(pb + off);
+}
+
+// atomicMin on a 16-bit entry (compare-and-swap on its 32-bit word); returns the old entry
+__device__ __forceinline__ uint32_t pmin(unsigned char *pb, uint32_t off, uint32_t val)
+{
+    uint32_t *word = reinterpret_cast<uint32_t *>(pb + (off & ~3u));
+    const uint32_t sh = (off & 2u) * 8u;
+    uint32_t old = *reinterpret_cast<volatile uint32_t *>(word);
+    for (;;) {
+        const uint32_t cur = (old >> sh) & 0xffffu;
+        if (cur <= val) return cur;
+        const uint32_t prev = atomicCAS(word, old, (old & ~(0xffffu << sh)) | (val << sh));
+        if (prev == old) return cur;
+        old = prev;
+    }
 }
 
 // find with path halving: every node on the way is re-pointed to its grandparent.  Racing writers
@@ -489,7 +506,7 @@ __device__ __forceinline__ uint32_t sfind_h(unsigned char *pb, uint32_t a)
     while (r != a) {
         const uint32_t g = pload(pb, r);
         if (g == r) return r;
-        *reinterpret_cast<volatile uint32_t *>(pb + a) = g;
+        *reinterpret_cast<volatile uint16_t *>(pb + a) = (uint16_t)g;
         a = g;
         r = pload(pb, a);
     }
@@ -504,7 +521,7 @@ __device__ __forceinline__ void sunion_v(unsigned char *pb, uint32_t a, uint32_t
         b = sfind_h(pb, b);
         if (a == b) return;
         const uint32_t hi = a > b ? a : b, lo = a > b ? b : a;
-        const uint32_t old = atomicMin(reinterpret_cast<uint32_t *>(pb + hi), lo);
+        const uint32_t old = pmin(pb, hi, lo);
         if (old == hi) return;
         a = old;                                   // hi was linked meanwhile: go on from its new parent
         b = lo;
@@ -519,12 +536,13 @@ k_label(const SweepArgs a)
     constexpr uint32_t LCAP = TW * TH / 2;           // entries of the wave lists: half the worst case (every y bond uniting)
     constexpr uint32_t NONE = 0xffffffffu;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    uint32_t *parent = reinterpret_cast<uint32_t *>(smem_raw);                       // [TW*TH]
-    uint32_t (*Xs)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 4);
-    uint32_t (*Ss)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 4);
-    uint32_t (*LLs)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 8);
-    uint16_t *wlist = reinterpret_cast<uint16_t *>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 12);           // per-wave lists of uniting y bonds (upper site)
-    uint32_t *wcnt = reinterpret_cast<uint32_t *>(smem_raw + (size_t)TW * TH * 4 + (size_t)TH * WPR * 12 + (size_t)TW * TH);   // [8] bonds in the list of wave j
+    static_assert(TW * TH <= 32768, "16-bit byte offsets");
+    uint16_t *parent = reinterpret_cast<uint16_t *>(smem_raw);                       // [TW*TH]
+    uint32_t (*Xs)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 2);
+    uint32_t (*Ss)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 2 + (size_t)TH * WPR * 4);
+    uint32_t (*LLs)[WPR] = reinterpret_cast<uint32_t (*)[WPR]>(smem_raw + (size_t)TW * TH * 2 + (size_t)TH * WPR * 8);
+    uint16_t *wlist = reinterpret_cast<uint16_t *>(smem_raw + (size_t)TW * TH * 2 + (size_t)TH * WPR * 12);           // per-wave lists of uniting y bonds (upper site)
+    uint32_t *wcnt = reinterpret_cast<uint32_t *>(smem_raw + (size_t)TW * TH * 2 + (size_t)TH * WPR * 12 + (size_t)TW * TH);   // [8] bonds in the list of wave j
 
     const uint32_t L = a.L;
     LabelT *labels = reinterpret_cast<LabelT *>(a.labels);
@@ -572,11 +590,11 @@ k_label(const SweepArgs a)
         const uint32_t wbase = row * TW + 32 * wq;
         const uint32_t m = Sq & ((2u << o) - 1u);
         uint4 st;
-        st.x = (m ? wbase + 31 - __clz(m) : LLs[row][wq]) * 4u;              // byte offsets (see pload)
-        st.y = ((Sq >> (o + 1)) & 1u) ? (wbase + o + 1) * 4u : st.x;
-        st.z = ((Sq >> (o + 2)) & 1u) ? (wbase + o + 2) * 4u : st.y;
-        st.w = ((Sq >> (o + 3)) & 1u) ? (wbase + o + 3) * 4u : st.z;
-        *reinterpret_cast<uint4 *>(&parent[wbase + o]) = st;
+        st.x = (m ? wbase + 31 - __clz(m) : LLs[row][wq]) * 2u;              // byte offsets (see pload)
+        st.y = ((Sq >> (o + 1)) & 1u) ? (wbase + o + 1) * 2u : st.x;
+        st.z = ((Sq >> (o + 2)) & 1u) ? (wbase + o + 2) * 2u : st.y;
+        st.w = ((Sq >> (o + 3)) & 1u) ? (wbase + o + 3) * 2u : st.z;
+        *reinterpret_cast<uint2 *>(&parent[wbase + o]) = make_uint2(st.x | (st.y << 16), st.z | (st.w << 16));
     }
 
     uint32_t need = 0;
@@ -608,7 +626,7 @@ k_label(const SweepArgs a)
     // it: either way a node of the right component to start the finds from
     unsigned char *pb = reinterpret_cast<unsigned char *>(parent);
     auto unite_at = [&](uint32_t site) {
-        sunion_v(pb, pload(pb, site * 4u), pload(pb, (site + TW) * 4u));
+        sunion_v(pb, pload(pb, site * 2u), pload(pb, (site + TW) * 2u));
     };
 #pragma unroll 1
     for (int j = 1; (1 << j) <= TH; ++j) {
@@ -633,10 +651,11 @@ k_label(const SweepArgs a)
 #pragma unroll 2
         for (int k = 0; k < TH / RPP; ++k) {
             const uint32_t i0 = (k * RPP + rq) * TW + 4 * q;
-            const uint4 p1 = *reinterpret_cast<const uint4 *>(&parent[i0]);
+            const uint2 w1 = *reinterpret_cast<const uint2 *>(&parent[i0]);
             uint4 p2;
-            p2.x = pload(pb, p1.x); p2.y = pload(pb, p1.y); p2.z = pload(pb, p1.z); p2.w = pload(pb, p1.w);
-            *reinterpret_cast<uint4 *>(&parent[i0]) = p2;
+            p2.x = pload(pb, w1.x & 0xffffu); p2.y = pload(pb, w1.x >> 16);
+            p2.z = pload(pb, w1.y & 0xffffu); p2.w = pload(pb, w1.y >> 16);
+            *reinterpret_cast<uint2 *>(&parent[i0]) = make_uint2(p2.x | (p2.y << 16), p2.z | (p2.w << 16));
         }
     }
 
@@ -646,8 +665,8 @@ k_label(const SweepArgs a)
     for (int k = 0; k < TH / RPP; ++k) {
         const int row = k * RPP + rq;
         const uint32_t i0 = row * TW + 4 * q;
-        const uint4 rt = *reinterpret_cast<const uint4 *>(&parent[i0]);
-        uint32_t root[4] = {rt.x, rt.y, rt.z, rt.w};
+        const uint2 rt = *reinterpret_cast<const uint2 *>(&parent[i0]);
+        uint32_t root[4] = {rt.x & 0xffffu, rt.x >> 16, rt.y & 0xffffu, rt.y >> 16};
         {
             uint32_t up[4];
 #pragma unroll
@@ -661,7 +680,7 @@ k_label(const SweepArgs a)
         uint32_t nib = 0;
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
-            const uint32_t rl = root[v] >> 2;                            // byte offset -> tile-local index
+            const uint32_t rl = root[v] >> 1;                            // byte offset -> tile-local index
             out[v] = gbase + (LabelT)(rl / TW) * L + (rl % TW);
             nib |= (rl == i0 + v) ? (1u << v) : 0u;
         }
