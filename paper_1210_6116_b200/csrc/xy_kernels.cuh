@@ -681,7 +681,7 @@ k_label(const SweepArgs a)
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
             const uint32_t rl = root[v] >> 1;                            // byte offset -> tile-local index
-            out[v] = gbase + (LabelT)(rl / TW) * L + (rl % TW);
+            out[v] = gbase + (LabelT)(rl / TW) * (L - TW) + rl;          // row * L + col with row * TW + col = rl
             nib |= (rl == i0 + v) ? (1u << v) : 0u;
         }
         const size_t gi = (size_t)(y0 + row) * L + x0 + 4 * q;
