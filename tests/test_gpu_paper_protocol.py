@@ -4,6 +4,8 @@
 error bars are for 4e6 MCS; ours are ~3.5 times wider.  Observed on the first run: beta_KT 1.09231 / 1.09808
 (paper 1.09167(25) / 1.09788(32)), <m^2> 0.34985 / 0.29574 (0.34924(29) / 0.29695(36)), xi_2nd/L 0.7484 /
 0.7474 (0.7464(11) / 0.7466(15)); the tolerances are about 3 of our standard errors."""
+import os
+
 import numpy as np
 import pytest
 
@@ -22,7 +24,12 @@ def xy():
     return m
 
 
-@pytest.mark.parametrize("L,seed", [(64, 21), (128, 22)])
+LONG = os.environ.get("XY_LONG") == "1"          # L = 1024 and 4096 take 20 s and 80 s of GPU time: opt-in
+
+
+@pytest.mark.parametrize("L,seed", [(64, 21), (128, 22),
+                                    pytest.param(1024, 23, marks=pytest.mark.skipif(not LONG, reason="set XY_LONG=1")),
+                                    pytest.param(4096, 24, marks=pytest.mark.skipif(not LONG, reason="set XY_LONG=1"))])
 def test_paper_protocol_table1(xy, L, seed):
     row = table1()[L]
     c = constants()
