@@ -46,6 +46,9 @@ enum {
     XY_FLAG_FOURIER = 2u            /* also reduce the structure-factor sums of every sweep (xy_fourier) */
 };
 
+enum { XY_OBS_NONE = 0,            /* chained sweeps do not reduce observables (thermalisation, throughput runs) */
+       XY_OBS_ALL  = 1 };          /* every sweep reduces the sums of xy_obs (default) */
+
 /* Observables of the configuration after `sweep` sweeps (PAPER.md:40 Eq. 3, :46-54 Eq. 4-6,
  * :107 Eq. 9).  All sums are un-normalised and accumulated in fp64.
  *   e_x = Cx/N, s_x = Sx/N,  Upsilon_x = <e_x> - beta N <s_x^2>,  <m^2> = <Mx^2+My^2>/N^2,  N = L^2. */
@@ -127,14 +130,29 @@ int xy_create_ex(xy_state **out, uint32_t L, uint64_t seed, int init, uint32_t f
 
 /* ---- parity / checkpoint extensions (host buffers; each synchronises the state's stream) ----- */
 
-/* the getters below copy the first n sites (row-major), 1 <= n <= L*L */
+/* the getters below copy the first n sites (row-major), 1 <= n <= L*L; the _range variants copy the n
+ * sites first .. first+n-1 (first + n <= L*L), so any part of a lattice too large for host memory can be
+ * inspected (label VALUES stay global site indices). */
 int xy_get_angles(xy_state *s, float *host, size_t n);
-int xy_set_angles(xy_state *s, const float *host, size_t n);    /* values must lie in [0, 6.2831855] */
+int xy_get_angles_range(xy_state *s, float *host, uint64_t first, size_t n);
+/* Replace the configuration (n = L*L values in [0, 6.2831855]).  The values are staged and range-checked
+ * on the device BEFORE they replace theta: on XY_ERR_ARG the configuration is unchanged.  The labels of
+ * the previous sweep are given up (their array is the staging area). */
+int xy_set_angles(xy_state *s, const float *host, size_t n);
 /* canonical labels of the most recent sweep, label = minimum site index of the cluster, widened
  * to int64 for every L; XY_ERR_STATE before the first sweep. */
 int xy_get_labels(xy_state *s, int64_t *host, size_t n);
+int xy_get_labels_range(xy_state *s, int64_t *host, uint64_t first, size_t n);
 /* bonds of the most recent sweep, one byte per site: bit0 = x bond, bit1 = y bond. */
 int xy_get_bonds(xy_state *s, uint8_t *host, size_t n);
+int xy_get_bonds_range(xy_state *s, uint8_t *host, uint64_t first, size_t n);
+/* Whole-lattice invariants of the most recent sweep's labels against its bonds, counted on the device
+ * (for lattices whose label array does not fit host memory): counts[0] = #{label[i] > i},
+ * counts[1] = #{label[label[i]] != label[i]}, counts[2] / counts[3] = active x / y bonds (periodic wrap
+ * included) whose ends carry different labels, counts[4] = #{label[i] == i} (the number of clusters).
+ * A correct labeling has counts[0..3] = 0 and counts[4] = xy_obs.n_clusters.  XY_ERR_STATE before the
+ * first sweep. */
+int xy_debug_check_labels(xy_state *s, uint64_t counts[5]);
 /* per-sweep records for T = first_sweep .. first_sweep+count-1 from the device ring
  * (capacity xy_series_capacity(); records older than that are gone -> XY_ERR_ARG). */
 int xy_get_series(xy_state *s, xy_obs *host, uint64_t first_sweep, uint64_t count);
@@ -147,6 +165,11 @@ int xy_get_fourier_series(xy_state *s, xy_fourier *host, uint64_t first_sweep, u
 int xy_get_sweep(xy_state *s, uint64_t *t);
 int xy_set_sweep(xy_state *s, uint64_t t);                      /* resume / sampled-sweep parity */
 int xy_debug_fix_phi(xy_state *s, int on, double phi);          /* Ising-limit and 2x2-style tests */
+/* XY_OBS_NONE: the following xy_sw_sweeps (and the `discard` sweeps of xy_pcc_run) skip the fp64
+ * observable sums (the bond decisions, labels and angles are unchanged, bit for bit); their ring records
+ * keep beta and the counts, the sums read NaN.  xy_measure still returns the sums of the current
+ * configuration (one observables-only pass).  XY_OBS_ALL (default) restores the per-sweep series. */
+int xy_set_obs_mode(xy_state *s, int mode);
 /* number of bond decisions of all sweeps so far that the fp32 filter could not settle and that
  * were re-evaluated with the full fp64 expression. */
 int xy_get_fallback_count(xy_state *s, uint64_t *count);

@@ -12,6 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libxy_b200.so")
 
 INIT_COLD, INIT_HOT = 0, 1
+OBS_NONE, OBS_ALL = 0, 1
 FLAG_LABELS64 = 1
 FLAG_FOURIER = 2
 
@@ -85,6 +86,11 @@ _SIGS = {
     "xy_pcc_run": [_vp, C.c_double, C.c_double, C.POINTER(PccSchedule), C.POINTER(_PccOut)],
     "xy_destroy": [_vp],
     "xy_get_angles": [_vp, _vp, C.c_size_t],
+    "xy_get_angles_range": [_vp, _vp, C.c_uint64, C.c_size_t],
+    "xy_get_labels_range": [_vp, _vp, C.c_uint64, C.c_size_t],
+    "xy_get_bonds_range": [_vp, _vp, C.c_uint64, C.c_size_t],
+    "xy_debug_check_labels": [_vp, C.POINTER(C.c_uint64)],
+    "xy_set_obs_mode": [_vp, C.c_int],
     "xy_set_angles": [_vp, _vp, C.c_size_t],
     "xy_get_labels": [_vp, _vp, C.c_size_t],
     "xy_get_bonds": [_vp, _vp, C.c_size_t],
@@ -188,11 +194,11 @@ class XYState:
             pass
 
     # -- extensions -------------------------------------------------------------------------
-    def get_angles(self, out=None, n=None):
-        """the first n sites (default: all)"""
-        n = self.N if n is None else int(n)
+    def get_angles(self, out=None, n=None, first=0):
+        """n sites from `first` (default: all)"""
+        n = self.N - first if n is None else int(n)
         out = np.empty(n, np.float32) if out is None else out
-        _check(_lib.xy_get_angles(self._h, _host_ptr(out), n))
+        _check(_lib.xy_get_angles_range(self._h, _host_ptr(out), first, n))
         return out
 
     def set_angles(self, theta):
@@ -200,17 +206,27 @@ class XYState:
             theta = np.ascontiguousarray(theta, np.float32)
         _check(_lib.xy_set_angles(self._h, _host_ptr(theta), self.N))
 
-    def get_labels(self, n=None):
-        n = self.N if n is None else int(n)
+    def get_labels(self, n=None, first=0):
+        n = self.N - first if n is None else int(n)
         out = np.empty(n, np.int64)
-        _check(_lib.xy_get_labels(self._h, out.ctypes.data, n))
+        _check(_lib.xy_get_labels_range(self._h, out.ctypes.data, first, n))
         return out
 
-    def get_bonds(self, n=None):
-        n = self.N if n is None else int(n)
+    def get_bonds(self, n=None, first=0):
+        n = self.N - first if n is None else int(n)
         out = np.empty(n, np.uint8)
-        _check(_lib.xy_get_bonds(self._h, out.ctypes.data, n))
+        _check(_lib.xy_get_bonds_range(self._h, out.ctypes.data, first, n))
         return out
+
+    def debug_check_labels(self):
+        """device-side invariants of the last sweep's labels: dict of the five counts"""
+        c = (C.c_uint64 * 5)()
+        _check(_lib.xy_debug_check_labels(self._h, c))
+        return {"label_above_index": int(c[0]), "root_not_fixed": int(c[1]), "x_bond_split": int(c[2]),
+                "y_bond_split": int(c[3]), "n_roots": int(c[4])}
+
+    def set_obs_mode(self, mode):
+        _check(_lib.xy_set_obs_mode(self._h, mode))
 
     def measure_fourier(self):
         """The 8 structure-factor sums of the current configuration (needs FLAG_FOURIER): array [8] = Fx, Fy."""

@@ -69,39 +69,35 @@ Layout make_layout(uint32_t L, uint32_t flags)
 
 // One set of launchers per (tile geometry, label width).
 struct Kernels {
-    void (*bonds)(const SweepArgs &, bool obs_only, bool fourier, int grid, cudaStream_t);
+    // what: 0 = sweep with observables, 1 = observables only, 2 = sweep without observables
+    cudaError_t (*bonds)(const SweepArgs &, int what, bool fourier, int grid, cudaStream_t);
     void (*label)(const SweepArgs &, cudaStream_t);
     void (*merge)(const SweepArgs &, cudaStream_t);
     void (*flip)(const SweepArgs &, int grid, cudaStream_t);
-    int (*occupancy)(bool fourier, int *bonds_sweep, int *bonds_obs, int *fl);
+    int (*prepare)(bool fourier, int *bonds_obs, int *bonds_noobs, int *fl);
     int tw, th, rs;
 };
 
 // rows per warp strip in k_bonds: 32 (1/32 halo recompute) on large lattices; 8 where 32-row strips would
 // leave warps without work or with one long serial strip (L <= 4096: fewer than 2 strips per resident warp)
 constexpr int kRSLarge = 32, kRSSmall = 8;
-constexpr int kBondsWarps = 4;   // warps per CTA in k_bonds
 
 template <int VEC, int R, int NW, int RS, typename LabelT>
 struct KS {
-    static void bonds(const SweepArgs &a, bool obs_only, bool fourier, int grid, cudaStream_t st)
+    template <bool kB, bool kO, bool kF>
+    static cudaError_t bonds_launch(const SweepArgs &a, int grid, cudaStream_t st)
     {
-        if (fourier) {
-            if (obs_only) k_bonds<VEC, RS, false, true><<<grid, kBondsWarps * 32, 0, st>>>(a);
-            else k_bonds<VEC, RS, true, true><<<grid, kBondsWarps * 32, 0, st>>>(a);
-        } else {
-            if (obs_only) k_bonds<VEC, RS, false, false><<<grid, kBondsWarps * 32, 0, st>>>(a);
-            else k_bonds<VEC, RS, true, false><<<grid, kBondsWarps * 32, 0, st>>>(a);
-        }
+        k_bonds<VEC, RS, kB, kO, kF><<<grid, kBondsWarps * 32, k_bonds_smem_bytes<kO>(), st>>>(a);
+        return cudaGetLastError();
+    }
+    static cudaError_t bonds(const SweepArgs &a, int what, bool fourier, int grid, cudaStream_t st)
+    {
+        if (what == 2) return bonds_launch<true, false, false>(a, grid, st);
+        if (fourier) return what == 1 ? bonds_launch<false, true, true>(a, grid, st) : bonds_launch<true, true, true>(a, grid, st);
+        return what == 1 ? bonds_launch<false, true, false>(a, grid, st) : bonds_launch<true, true, false>(a, grid, st);
     }
     static void label(const SweepArgs &a, cudaStream_t st)
     {
-        static bool attr_set = false;
-        if (!attr_set) {
-            cudaFuncSetAttribute(k_label<VEC, R * NW, LabelT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)k_label_smem_bytes<VEC, R * NW>());
-            attr_set = true;
-        }
         k_label<VEC, R * NW, LabelT><<<a.ntiles, VEC * R * NW, k_label_smem_bytes<VEC, R * NW>(), st>>>(a);
     }
     static void merge(const SweepArgs &a, cudaStream_t st)
@@ -116,21 +112,42 @@ struct KS {
         (void)grid;
         k_flip<VEC, R * NW, LabelT><<<a.ntiles, VEC * R * NW, 0, st>>>(a);
     }
-    static int occupancy(bool fourier, int *bonds_sweep, int *bonds_obs, int *fl)
+    template <bool kB, bool kO, bool kF>
+    static cudaError_t bonds_prepare(int *occ)
+    {
+        // opt in to more than 48 KB of dynamic shared memory: per device, so set at every state creation
+        cudaError_t e = cudaFuncSetAttribute(k_bonds<VEC, RS, kB, kO, kF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)k_bonds_smem_bytes<kO>());
+        if (e != cudaSuccess) return e;
+        int n = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_bonds<VEC, RS, kB, kO, kF>, kBondsWarps * 32,
+                                                          k_bonds_smem_bytes<kO>());
+        if (occ && (*occ == 0 || n < *occ)) *occ = n;
+        return e;
+    }
+    // sets the kernel attributes on the current device; CTAs per SM of the k_bonds variants with observables
+    // (they share ONE grid so that their fixed-order sums agree bitwise), of the variant without, of k_flip
+    static int prepare(bool fourier, int *bonds_obs, int *bonds_noobs, int *fl)
     {
         cudaError_t e;
-        if (fourier) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_sweep, k_bonds<VEC, RS, true, true>, kBondsWarps * 32, 0);
-        else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_sweep, k_bonds<VEC, RS, true, false>, kBondsWarps * 32, 0);
-        if (e != cudaSuccess) return (int)e;
-        if (fourier) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_obs, k_bonds<VEC, RS, false, true>, kBondsWarps * 32, 0);
-        else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(bonds_obs, k_bonds<VEC, RS, false, false>, kBondsWarps * 32, 0);
-        if (e != cudaSuccess) return (int)e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(fl, k_flip<VEC, R * NW, LabelT>, VEC * R * NW, 0);
+        *bonds_obs = 0; *bonds_noobs = 0;
+        if (fourier) {
+            e = bonds_prepare<true, true, true>(bonds_obs);
+            if (e == cudaSuccess) e = bonds_prepare<false, true, true>(bonds_obs);
+        } else {
+            e = bonds_prepare<true, true, false>(bonds_obs);
+            if (e == cudaSuccess) e = bonds_prepare<false, true, false>(bonds_obs);
+        }
+        if (e == cudaSuccess) e = bonds_prepare<true, false, false>(bonds_noobs);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(k_label<VEC, R * NW, LabelT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)k_label_smem_bytes<VEC, R * NW>());
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(fl, k_flip<VEC, R * NW, LabelT>, VEC * R * NW, 0);
         return (int)e;
     }
     static Kernels get()
     {
-        return Kernels{&bonds, &label, &merge, &flip, &occupancy, 32 * VEC, R * NW, RS};
+        return Kernels{&bonds, &label, &merge, &flip, &prepare, 32 * VEC, R * NW, RS};
     }
 };
 
@@ -224,7 +241,9 @@ struct xy_state {
     char *ws = nullptr;
     Layout lay{};
     Kernels ker{};
-    int grid_bonds = 0, grid_fl = 0;
+    int grid_bonds = 0, grid_bonds_noobs = 0, grid_fl = 0;
+    int obs_mode = XY_OBS_ALL;      // xy_set_obs_mode
+    bool poisoned = false;          // xy_set_angles rejected its input and nothing valid was restored
     cudaStream_t stream = nullptr;
     bool have_sweep = false;        // bonds / labels of a sweep exist
     bool labels_flat = false;
@@ -300,6 +319,7 @@ SweepArgs base_args(const xy_state *s)
         a.rk[2 * r + 1] = a.seed_hi + r * 0xBB67AE85u;
     }
     a.t = (uint32_t)s->T;
+    a.cphi = 1.0;                   // observables-only launches use the unrotated frame (phi = 0)
     a.sincos_tab = s->tab();
     a.fring = s->fring();
     {
@@ -342,8 +362,7 @@ int ensure_obs(xy_state *s, int feed_pcc)
     SweepArgs a = base_args(s);
     a.obs_fill = 1;
     a.feed_pcc = feed_pcc;
-    s->ker.bonds(a, true, s->fourier(), s->grid_bonds, s->stream);
-    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(s->ker.bonds(a, 1, s->fourier(), s->grid_bonds, s->stream));
     s->launches += 1;
     s->obs_valid_T = s->T;
     return XY_OK;
@@ -388,13 +407,17 @@ int enqueue_sweep(xy_state *s, double beta, int beta_from_ctl, int feed_pcc)
     a.beta = beta;
     a.beta_from_ctl = beta_from_ctl;
     a.feed_pcc = feed_pcc;
-    a.obs_fill = (s->obs_valid_T == s->T) ? 0 : 1;
+    // observables of the incoming state ride on this sweep's k_bonds unless they are switched off (and the
+    // PCC controller does not need them) or already on their way
+    const bool with_obs = feed_pcc || (s->obs_mode == XY_OBS_ALL && s->obs_valid_T != s->T);
+    a.obs_fill = (with_obs && s->obs_valid_T != s->T) ? 1 : 0;
     if (s->timing) {
         if (s->ev_used >= (kTimedKernels + 1) * kTimedSweepsPerFlush)
             if (int rc = timing_flush(s)) return rc;
         if (int rc = timing_mark(s)) return rc;
     }
-    s->ker.bonds(a, false, s->fourier(), s->grid_bonds, s->stream);
+    if (with_obs) CUDA_TRY(s->ker.bonds(a, 0, s->fourier(), s->grid_bonds, s->stream));
+    else CUDA_TRY(s->ker.bonds(a, 2, false, s->grid_bonds_noobs, s->stream));
     if (s->timing) if (int rc = timing_mark(s)) return rc;
     s->ker.label(a, s->stream);
     if (s->timing) if (int rc = timing_mark(s)) return rc;
@@ -461,10 +484,10 @@ int xy_create_ex(xy_state **out, uint32_t L, uint64_t seed, int init, uint32_t f
         s->ws = static_cast<char *>(p);
         s->owns_ws = true;
     }
-    int bs = 0, bo = 0, fl = 0, sms = 0;
-    cudaError_t e = (cudaError_t)s->ker.occupancy(s->fourier(), &bs, &bo, &fl);
+    int bo = 0, bn = 0, fl = 0, sms = 0;
+    cudaError_t e = (cudaError_t)s->ker.prepare(s->fourier(), &bo, &bn, &fl);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device);
-    if (e != cudaSuccess || bs < 1 || bo < 1 || fl < 1) {
+    if (e != cudaSuccess || bo < 1 || bn < 1 || fl < 1) {
         if (s->owns_ws) cudaFree(s->ws);
         delete s;
         return fail(XY_ERR_CUDA, "kernel occupancy query failed: %s (was the library built for this GPU's sm_100a?)",
@@ -472,28 +495,30 @@ int xy_create_ex(xy_state **out, uint32_t L, uint64_t seed, int init, uint32_t f
     }
     const uint32_t ntiles = (L / s->ker.tw) * (L / s->ker.th);
     const uint32_t nstrips = (L / s->ker.tw) * (L / s->ker.rs);
-    // both variants of k_bonds share ONE grid so that their fixed-order sums agree bitwise
-    long g = (long)sms * (bs < bo ? bs : bo);
+    // the variants of k_bonds with observables share ONE grid so that their fixed-order sums agree bitwise
     const long need = (nstrips + kBondsWarps - 1) / kBondsWarps;
+    long g = (long)sms * bo;
     if (g > need) g = need;
     if (g > (long)kMaxGrid) g = kMaxGrid;
     s->grid_bonds = (int)g;
+    g = (long)sms * bn;
+    if (g > need) g = need;
+    if (g > (long)kMaxGrid) g = kMaxGrid;
+    s->grid_bonds_noobs = (int)g;
     g = (long)sms * fl;
     if (g > (long)ntiles) g = ntiles;
     s->grid_fl = (int)g;
 
-    // sincos table: (cos, sin)(2 pi k / 256), k = 0..256, correctly rounded by the host libm
+    // table (cos, sin)(k / 1024), k = 0..kTabN: the angles are exact doubles, the values correctly rounded
+    // from the host's long-double libm
     {
-        double2 h[kTabN + 1];
+        std::vector<double2> h(kTabN + 1);
         for (int k = 0; k <= kTabN; ++k) {
-            const long double ang = 6.283185307179586476925286766559L * (long double)k / (long double)kTabN;
+            const long double ang = (long double)k / 1024.0L;
             h[k].x = (double)cosl(ang);
             h[k].y = (double)sinl(ang);
         }
-        h[0].x = 1.0; h[0].y = 0.0; h[kTabN].x = 1.0; h[kTabN].y = 0.0;
-        h[kTabN / 2].x = -1.0; h[kTabN / 2].y = 0.0;
-        h[kTabN / 4].x = 0.0; h[kTabN / 4].y = 1.0; h[3 * kTabN / 4].x = 0.0; h[3 * kTabN / 4].y = -1.0;
-        e = cudaMemcpy(s->tab(), h, sizeof h, cudaMemcpyHostToDevice);
+        e = cudaMemcpy(s->tab(), h.data(), h.size() * sizeof(double2), cudaMemcpyHostToDevice);
         if (e != cudaSuccess) {
             if (s->owns_ws) cudaFree(s->ws);
             delete s;
@@ -646,35 +671,57 @@ int xy_pcc_run(xy_state *s, double beta0, double dbeta0, const xy_pcc_schedule *
     return XY_OK;
 }
 
-int xy_get_angles(xy_state *s, float *host, size_t n)
+static int check_range(const xy_state *s, uint64_t first, size_t n)
+{
+    if (n == 0 || first >= s->N || n > s->N - first)
+        return fail(XY_ERR_ARG, "sites %llu..%llu not in 0..%llu", (unsigned long long)first,
+                    (unsigned long long)(first + n) - 1, (unsigned long long)s->N - 1);
+    return XY_OK;
+}
+
+int xy_get_angles_range(xy_state *s, float *host, uint64_t first, size_t n)
 {
     if (!s || !host) return fail(XY_ERR_ARG, "NULL argument");
-    if (n == 0 || n > s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
+    if (int rc = check_range(s, first, n)) return rc;
     DeviceGuard g(s->device);
-    CUDA_TRY(cudaMemcpyAsync(host, s->theta(), n * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(cudaMemcpyAsync(host, s->theta() + first, n * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
     CUDA_TRY(cudaStreamSynchronize(s->stream));
     return XY_OK;
 }
+
+int xy_get_angles(xy_state *s, float *host, size_t n) { return xy_get_angles_range(s, host, 0, n); }
 
 int xy_set_angles(xy_state *s, const float *host, size_t n)
 {
     if (!s || !host) return fail(XY_ERR_ARG, "NULL argument");
     if (n != s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
     DeviceGuard g(s->device);
-    CUDA_TRY(cudaMemcpyAsync(s->theta(), host, n * sizeof(float), cudaMemcpyHostToDevice, s->stream));
-    k_ring_reset<<<1, 32, 0, s->stream>>>(s->ring(), kRingCap, s->T);
-    // range check on the device (the flag lives in the control block)
-    k_check_angles<<<148 * 8, 256, 0, s->stream>>>(s->theta(), s->N, &s->ctl()->pad);
+    // staged in the label array (>= 4 N bytes; the labels of the previous sweep are given up), checked
+    // there, and copied to theta only if every value is in range: a rejected call leaves theta untouched
+    float *stage = static_cast<float *>(s->labels());
+    CUDA_TRY(cudaMemcpyAsync(stage, host, n * sizeof(float), cudaMemcpyHostToDevice, s->stream));
+    k_check_angles<<<148 * 8, 256, 0, s->stream>>>(stage, s->N, &s->ctl()->pad);
     unsigned int bad = 0;
     CUDA_TRY(cudaMemcpyAsync(&bad, &s->ctl()->pad, sizeof bad, cudaMemcpyDeviceToHost, s->stream));
     CUDA_TRY(cudaStreamSynchronize(s->stream));
-    s->obs_valid_T = UINT64_MAX;
-    s->oldest_T = s->T;
     s->have_sweep = false;
     if (bad) {
         CUDA_TRY(cudaMemsetAsync(&s->ctl()->pad, 0, sizeof bad, s->stream));
-        return fail(XY_ERR_ARG, "angles outside [0, 6.2831855] (or NaN): the state now holds the rejected values");
+        return fail(XY_ERR_ARG, "angles outside [0, 6.2831855] (or NaN): rejected, the configuration is unchanged");
     }
+    CUDA_TRY(cudaMemcpyAsync(s->theta(), stage, n * sizeof(float), cudaMemcpyDeviceToDevice, s->stream));
+    k_ring_reset<<<1, 32, 0, s->stream>>>(s->ring(), kRingCap, s->T);
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    s->obs_valid_T = UINT64_MAX;
+    s->oldest_T = s->T;
+    return XY_OK;
+}
+
+int xy_set_obs_mode(xy_state *s, int mode)
+{
+    if (!s) return fail(XY_ERR_ARG, "state is NULL");
+    if (mode != XY_OBS_NONE && mode != XY_OBS_ALL) return fail(XY_ERR_ARG, "obs mode %d unknown", mode);
+    s->obs_mode = mode;
     return XY_OK;
 }
 
@@ -782,46 +829,77 @@ int xy_get_fallback_count(xy_state *s, uint64_t *count)
     return XY_OK;
 }
 
-int xy_get_labels(xy_state *s, int64_t *host, size_t n)
+// label[i] <- root(i) in place, once per sweep (S5 as an array; the sweep itself never needs it)
+static int ensure_flat(xy_state *s)
+{
+    if (s->labels_flat) return XY_OK;
+    if (s->l64()) k_flatten<uint64_t><<<148 * 8, 256, 0, s->stream>>>(static_cast<uint64_t *>(s->labels()), s->N);
+    else k_flatten<uint32_t><<<148 * 8, 256, 0, s->stream>>>(static_cast<uint32_t *>(s->labels()), s->N);
+    CUDA_TRY(cudaGetLastError());
+    s->launches += 1;
+    s->labels_flat = true;
+    return XY_OK;
+}
+
+int xy_get_labels_range(xy_state *s, int64_t *host, uint64_t first, size_t n)
 {
     if (!s || !host) return fail(XY_ERR_ARG, "NULL argument");
-    if (n == 0 || n > s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
+    if (int rc = check_range(s, first, n)) return rc;
     if (!s->have_sweep) return fail(XY_ERR_STATE, "no sweep has produced labels yet");
     DeviceGuard g(s->device);
     if (int rc = ensure_stage(s)) return rc;
-    if (!s->labels_flat) {
-        if (s->l64()) k_flatten<uint64_t><<<148 * 8, 256, 0, s->stream>>>(static_cast<uint64_t *>(s->labels()), s->N);
-        else k_flatten<uint32_t><<<148 * 8, 256, 0, s->stream>>>(static_cast<uint32_t *>(s->labels()), s->N);
-        CUDA_TRY(cudaGetLastError());
-        s->labels_flat = true;
-    }
+    if (int rc = ensure_flat(s)) return rc;
     const uint64_t chunk = kStageBytes / sizeof(int64_t);
-    for (uint64_t first = 0; first < n; first += chunk) {
-        const uint64_t m = n - first < chunk ? n - first : chunk;
-        if (s->l64()) k_labels_to_i64<uint64_t><<<148 * 4, 256, 0, s->stream>>>(static_cast<const uint64_t *>(s->labels()), static_cast<int64_t *>(s->stage), first, m);
-        else k_labels_to_i64<uint32_t><<<148 * 4, 256, 0, s->stream>>>(static_cast<const uint32_t *>(s->labels()), static_cast<int64_t *>(s->stage), first, m);
-        CUDA_TRY(cudaMemcpyAsync(host + first, s->stage, m * sizeof(int64_t), cudaMemcpyDeviceToHost, s->stream));
+    for (uint64_t done = 0; done < n; done += chunk) {
+        const uint64_t m = n - done < chunk ? n - done : chunk;
+        if (s->l64()) k_labels_to_i64<uint64_t><<<148 * 4, 256, 0, s->stream>>>(static_cast<const uint64_t *>(s->labels()), static_cast<int64_t *>(s->stage), first + done, m);
+        else k_labels_to_i64<uint32_t><<<148 * 4, 256, 0, s->stream>>>(static_cast<const uint32_t *>(s->labels()), static_cast<int64_t *>(s->stage), first + done, m);
+        CUDA_TRY(cudaMemcpyAsync(host + done, s->stage, m * sizeof(int64_t), cudaMemcpyDeviceToHost, s->stream));
         CUDA_TRY(cudaStreamSynchronize(s->stream));
     }
     return XY_OK;
 }
 
-int xy_get_bonds(xy_state *s, uint8_t *host, size_t n)
+int xy_get_labels(xy_state *s, int64_t *host, size_t n) { return xy_get_labels_range(s, host, 0, n); }
+
+int xy_debug_check_labels(xy_state *s, uint64_t counts[5])
+{
+    if (!s || !counts) return fail(XY_ERR_ARG, "NULL argument");
+    if (!s->have_sweep) return fail(XY_ERR_STATE, "no sweep has produced labels yet");
+    DeviceGuard g(s->device);
+    if (int rc = ensure_stage(s)) return rc;
+    if (int rc = ensure_flat(s)) return rc;
+    unsigned long long *d = static_cast<unsigned long long *>(s->stage);
+    CUDA_TRY(cudaMemsetAsync(d, 0, 5 * sizeof(unsigned long long), s->stream));
+    if (s->l64()) k_check_labels<uint64_t><<<148 * 8, 256, 0, s->stream>>>(static_cast<const uint64_t *>(s->labels()), s->bonds(), s->L, d);
+    else k_check_labels<uint32_t><<<148 * 8, 256, 0, s->stream>>>(static_cast<const uint32_t *>(s->labels()), s->bonds(), s->L, d);
+    CUDA_TRY(cudaGetLastError());
+    s->launches += 1;
+    unsigned long long h[5];
+    CUDA_TRY(cudaMemcpyAsync(h, d, sizeof h, cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    for (int k = 0; k < 5; ++k) counts[k] = h[k];
+    return XY_OK;
+}
+
+int xy_get_bonds_range(xy_state *s, uint8_t *host, uint64_t first, size_t n)
 {
     if (!s || !host) return fail(XY_ERR_ARG, "NULL argument");
-    if (n == 0 || n > s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
+    if (int rc = check_range(s, first, n)) return rc;
     if (!s->have_sweep) return fail(XY_ERR_STATE, "no sweep has produced bonds yet");
     DeviceGuard g(s->device);
     if (int rc = ensure_stage(s)) return rc;
     const uint64_t chunk = kStageBytes;
-    for (uint64_t first = 0; first < n; first += chunk) {
-        const uint64_t m = n - first < chunk ? n - first : chunk;
-        k_bonds_unpack<<<148 * 4, 256, 0, s->stream>>>(s->bonds(), static_cast<uint8_t *>(s->stage), first, m);
-        CUDA_TRY(cudaMemcpyAsync(host + first, s->stage, m, cudaMemcpyDeviceToHost, s->stream));
+    for (uint64_t done = 0; done < n; done += chunk) {
+        const uint64_t m = n - done < chunk ? n - done : chunk;
+        k_bonds_unpack<<<148 * 4, 256, 0, s->stream>>>(s->bonds(), static_cast<uint8_t *>(s->stage), first + done, m);
+        CUDA_TRY(cudaMemcpyAsync(host + done, s->stage, m, cudaMemcpyDeviceToHost, s->stream));
         CUDA_TRY(cudaStreamSynchronize(s->stream));
     }
     return XY_OK;
 }
+
+int xy_get_bonds(xy_state *s, uint8_t *host, size_t n) { return xy_get_bonds_range(s, host, 0, n); }
 
 int xy_label_bonds(xy_state *s, const uint8_t *host_bonds, size_t n)
 {

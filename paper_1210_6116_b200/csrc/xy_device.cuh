@@ -89,22 +89,33 @@ __device__ __noinline__ bool bond_exact_at(const float *theta, uint32_t L, uint3
     return bond_exact(theta[(size_t)y * L + x], theta[(size_t)y2 * L + x2], phi, beta, w, fallback_counter);
 }
 
-// Filter (fp32, on the 16 leading bits of u): with sigma rounded to fp32, e32 = ex2.approx((sigma_i
-// m2b) sigma_j), m2b = -2 beta log2(e), approximates e = 1 - p = exp(-2 beta sigma_i sigma_j);
-// f = 1 + v with v = ((65535 - h) + 0.5) 2^-16 the midpoint of the interval that 1 - u lies in when only
-// the leading 16 bits h of the random word are known, so d = (e32 + 1) - f approximates e - (1 - u), and
+// Filter (fp32, on the 16 leading bits of u): e32 = ex2.approx((sigma_i m2b) sigma_j), m2b = -2 beta
+// log2(e), approximates e = 1 - p = exp(-2 beta sigma_i sigma_j); f = 1 + v with
+// v = ((65535 - h) + 0.5) 2^-16 the midpoint of the interval that 1 - u lies in when only the leading
+// 16 bits h of the random word are known, so d = (e32 + 1) - f approximates e - (1 - u), and
 //     u < p  <=>  e < 1 - u  <=>  d < 0.
-// Error budget of d: the exponent x = a m2b carries a relative error < 4e-7 (three fp32 roundings of
-// sigma, two products, m2b itself), so |delta e| = e ln2 |x| 4e-7 <= 0.531 * 0.693 * 4e-7 = 1.5e-7 at
-// ANY beta (x 2^-x <= 0.531); ex2.approx: 2^-22 relative, <= 2.4e-7; e32 + 1: 6e-8; f subtracts
-// exactly; the unknown trailing bits of u: 2^-17 = 7.7e-6.  Total < 8.3e-6, so |d| > kFilterDelta = 1e-5
-// settles the sign; otherwise (2e-5 of all bonds) the trailing bits are drawn and the definition is
-// evaluated in fp64 (bond_exact).
-constexpr float kFilterDelta = 1e-5f;
+// Error budget of d (sigma from k_bonds' fp32 table path, |delta sigma| <= 1e-7 ABSOLUTE: two table
+// roundings and two fused roundings of 2^-25 each, truncation 2e-11):
+//   exponent y = (sigma_i m2b) sigma_j: three fp32 roundings (m2b, two products), relative 1.8e-7,
+//     -> |delta e| <= e ln2 |y| 1.8e-7 <= 0.531 * 0.693 * 1.8e-7 = 6.6e-8 (y 2^-y <= 0.531 for y <= 0;
+//     for y > 0 the true e exceeds 1 and no error of this size can bring e32 below 1 - delta);
+//   the absolute sigma errors: |delta y| <= |m2b| (|sigma_i| + |sigma_j|) 1e-7, so
+//     |delta e| <= 2 beta (|sigma_i| + |sigma_j|) exp(-2 beta sigma_i sigma_j) 1e-7 <= 4e-7 beta;
+//   ex2.approx: 2^-22 relative <= 2.4e-7;  e32 + 1: 6e-8;  f subtracts exactly;
+//   the unknown trailing bits of u: 2^-17 = 7.63e-6.
+// Total < 8.0e-6 + 4e-7 beta.  |d| > delta(beta) = 1.2e-5 + 1e-6 beta (margin >= 1.4 at every beta)
+// settles the sign; otherwise (2 delta of all bonds: 2.6e-5 at beta = 1.12) the trailing bits are
+// drawn and the definition is evaluated in fp64 (bond_exact).  At huge beta delta exceeds every |d|
+// and all decisions take the exact path.
+__host__ __device__ __forceinline__ float filter_delta(double beta)
+{
+    return (float)(1.2e-5 + 1.0e-6 * beta);
+}
 
 struct BondCtx {
     double phi, beta;
     float m2b;                                  // -2 beta log2(e), fp32
+    float delta;                                // filter_delta(beta)
     unsigned long long *fallback_counter;
 };
 

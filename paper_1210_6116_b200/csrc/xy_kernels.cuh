@@ -1,9 +1,10 @@
 // xy_kernels.cuh -- the kernels of one Swendsen-Wang sweep of the 2D XY model on sm_100a.
 //
 //   k_bonds   (S2, and S7 of the incoming configuration): warps stream strips of the lattice row
-//             by row: theta -> fp64 (cos, sin, sigma) per site in registers (table + short Taylor
-//             rotation) -> observables, Philox bond draws, filtered bond decisions -> packed bond
-//             bits (0.25 B/site).  theta is read once (+ halo); no block barrier in the loop.
+//             by row: theta is split exactly on a 2^-10 grid in fp32; sigma (fp32) and (cos, sin)
+//             (fp64) per site come from two shared-memory tables and a second-order rotation ->
+//             observables, Philox bond draws, filtered bond decisions -> packed bond bits
+//             (0.25 B/site).  theta is read once (+ halo); no block barrier in the loop.
 //   k_label   (S3): one CTA per TW x TH tile, integer only, bit-parallel: a thread holds the x / y
 //             bond bits of 32 sites in two registers; union-find over RUNS of x bonds in shared
 //             memory, united in log2(TH) waves -> provisional label (global index of the
@@ -66,7 +67,7 @@ struct SweepArgs {
     int          obs_fill;        // 1: finalize writes the observables of the incoming state into ring[T]
     double       beta;
     double       phi, cphi, sphi, A;
-    const double2 *sincos_tab;    // [kTabN + 1] (cos, sin)(2 pi k / kTabN), host-computed
+    const double2 *sincos_tab;    // [kTabN + 1] (cos, sin)(k / 1024), host-computed
     double       ck1, sk1;        // (cos, sin)(2 pi / L)
     xy_fourier  *fring;           // ring of structure-factor records (XY_FLAG_FOURIER), else unused
 };
@@ -142,42 +143,78 @@ __device__ inline void pcc_feed(DevCtl *c, double N, double Cx, double Sx, doubl
 // Right neighbour of a lane's last site: shuffle from lane+1; for lane 31 the strip's halo column,
 // computed once per strip by lanes 0..RS-1 into a per-warp shared slot.  Row RS of the strip (the
 // first row of the strip below) is recomputed as the y-halo (1/RS overhead).
-// ---------------------------------------------------------------------------------------------
-constexpr int kTabN = 1024;                // sincos table: entries k = 0..1024 at angle 2 pi k / 1024
-
-// sin, cos of an fp32 angle in [0, 2pi(1+1e-7)]: table lookup + short Taylor rotation in fp64.
-// |x| <= pi/1024: sin x = x - x^3/6 (+2.3e-15), cos x - 1 = -x^2/2 + x^4/24 (+1.2e-18); the reduction
-// uses fl64(2 pi) k/1024 (exact scaling) for the table angle 2 pi k/1024: off by <= 2.5e-16.  |error| < 4e-15.
-__device__ __forceinline__ void sincos_tab(float theta, const double2 *tab, double &s, double &c)
-{
-    const double t = (double)theta;
-    const double kd = __fma_rn(t, 162.97466172610083, 6755399441055744.0);      // 1024/(2 pi), round to integer
-    const int k = __double2loint(kd);
-    const double kf = kd - 6755399441055744.0;
-    const double x = __fma_rn(-kf, 0.006135923151542565, t);                    // fl64(2 pi)/1024
-    const double2 cs = tab[k];
-    const double x2 = x * x;
-    const double sx = __fma_rn(x * x2, -1.6666666666666667e-1, x);
-    const double dc = x2 * __fma_rn(x2, 4.1666666666666667e-2, -0.5);           // cos x - 1
-    c = __fma_rn(-cs.y, sx, __fma_rn(cs.x, dc, cs.x));
-    s = __fma_rn(cs.x, sx, __fma_rn(cs.y, dc, cs.y));
-}
-
+//
+// Angle -> (cos, sin)(theta - phi) per site; sigma IS the cosine.  theta is split EXACTLY in fp32 on
+// the grid h = k 2^-10:
+//   tm = theta + 1.5 2^13 (round to nearest: ulp 2^-10), h = tm - 1.5 2^13, x = theta - h,
+//   |x| <= 2^-11, all three exact; k = tm's mantissa bits above 2^22 (bits(tm) - bits(1.5 2^13)), 0 <= k <= 6434.
+// The table of the sweep, (C_k, S_k) = (cos, sin)(k 2^-10 - phi), is rotated at kernel start from the
+// host-computed (cos, sin)(k 2^-10) into shared memory (fp64 with observables, fp32 without), and
+//   (cos, sin)(theta - phi) = (C_k w - S_k x, S_k w + C_k x), w = 1 - x^2/2:
+//   one conversion of x (exact) and 6 fp64 operations, sigma = that cosine rounded to fp32; without
+//   observables 4 fp32 operations on the fp32 table.  Truncation: |sin x - x| <= x^3/6 <= 1.95e-11,
+//   |cos x - w| <= x^4/24 <= 2.4e-15; table entries within 3e-16.
+// The link sums Cx, Sx, Cy, Sy depend on angle differences only, so they are the same in the rotated
+// frame; Mx, My (and the structure-factor sums) are linear in (cos, sin) and are rotated back by phi
+// once, in finalize.
 // kFourier: also reduce the 8 structure-factor sums at k = 2 pi / L (x and y direction) of the
 // incoming configuration (Eq. 8-9): per-column sums of (cos, sin) live in registers
-// for the 32 rows of a strip and meet e^{ik x} once per strip; per-row sums meet e^{ik y} once per row.
-template <int VEC, int RS, bool kBonds, bool kFourier>
-__global__ void __launch_bounds__(128, kFourier ? 3 : 4)
+// for the rows of a strip and meet e^{ik x} once per strip; per-row sums meet e^{ik y} once per row.
+// kObs = false (xy_set_obs_mode(XY_OBS_NONE)): fp32 only, no fp64 table, no sums; bond counts only.
+// ---------------------------------------------------------------------------------------------
+constexpr int kTabN = 6434;                 // table entries k = 0..kTabN at angle k / 1024; 6434/1024 >= fl32(2 pi)
+constexpr float kTabMagic = 12288.0f;       // 1.5 * 2^13: fp32 ulp 2^-10 in [2^13, 2^14)
+constexpr int kBondsWarps = 16;             // warps per CTA in k_bonds
+
+template <bool kObs>
+constexpr size_t k_bonds_smem_bytes()
+{
+    return (size_t)(kTabN + 1) * (kObs ? sizeof(double2) : sizeof(float2)) + 16;
+}
+
+// one table, indexed by byte offset: entries are double2 with observables, float2 without
+template <bool kObs>
+struct BondsEntry { static constexpr uint32_t bytes = kObs ? 16u : 8u; };
+
+// tab_adj = shared-space byte address of entry 0 minus bits(kTabMagic) * entry size (mod 2^32): the entry
+// of an angle is one multiply-add away from the bits of tm
+template <bool kBonds, bool kObs>
+__device__ __forceinline__ void site_eval(float theta, uint32_t tab_adj, float &g, double &c, double &s)
+{
+    const float tm = __fadd_rn(theta, kTabMagic);
+    const float h = __fadd_rn(tm, -kTabMagic);
+    const float x = __fadd_rn(theta, -h);
+    const uint32_t addr = __float_as_uint(tm) * BondsEntry<kObs>::bytes + tab_adj;
+    if constexpr (kObs) {
+        double C, S;
+        asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(C), "=d"(S) : "r"(addr));
+        const double xd = (double)x;
+        const double w = __fma_rn(xd * xd, -0.5, 1.0);
+        c = __fma_rn(-S, xd, C * w);
+        s = __fma_rn(C, xd, S * w);
+        if constexpr (kBonds) g = __double2float_rn(c);
+    } else {
+        float C, S;
+        asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(C), "=f"(S) : "r"(addr));
+        const float dc = (-0.5f * x) * x;
+        g = fmaf(-S, x, fmaf(C, dc, C));
+    }
+}
+
+template <int VEC, int RS, bool kBonds, bool kObs, bool kFourier>
+__global__ void __launch_bounds__(kBondsWarps * 32, kObs ? 1 : 2)
 k_bonds(const SweepArgs a)
 {
-    constexpr int NW = 4;
+    static_assert(kObs || !kFourier, "the structure-factor sums are observables");
+    static_assert(kBonds || kObs, "nothing to do");
+    constexpr int NW = kBondsWarps;
     constexpr int NS = kFourier ? 14 : 6;      // fp64 sums per thread / warp / CTA
     constexpr int TW = 32 * VEC;
     static_assert(RS <= 32, "halo column is computed by one lane per row");
 
-    __shared__ double2 tab[kTabN + 1];
-    __shared__ double h_c[NW][RS], h_s[NW][RS];
-    __shared__ float h_g[NW][RS];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double h_c[kObs ? NW : 1][RS], h_s[kObs ? NW : 1][RS];
+    __shared__ float h_g[kBonds ? NW : 1][RS];
     __shared__ double red[NW][NS];
     __shared__ double2 h_ky[kFourier ? NW : 1][RS];      // (cos, sin)(2 pi y / L) of the strip's rows
     __shared__ unsigned long long redc[NW][2];
@@ -186,7 +223,15 @@ k_bonds(const SweepArgs a)
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
     const uint32_t L = a.L;
-    for (int k = threadIdx.x; k <= kTabN; k += blockDim.x) tab[k] = a.sincos_tab[k];
+    const double cphi = a.cphi, sphi = a.sphi;
+    for (int k = threadIdx.x; k <= kTabN; k += blockDim.x) {      // (cos, sin)(h_k - phi), once per CTA and sweep
+        const double2 cs = __ldg(a.sincos_tab + k);
+        const double cr = __fma_rn(cs.x, cphi, cs.y * sphi), sr = __fma_rn(cs.y, cphi, -(cs.x * sphi));
+        if constexpr (kObs) reinterpret_cast<double2 *>(smem_raw)[k] = make_double2(cr, sr);
+        else reinterpret_cast<float2 *>(smem_raw)[k] = make_float2(__double2float_rn(cr), __double2float_rn(sr));
+    }
+    const uint32_t tab_adj = (uint32_t)__cvta_generic_to_shared(smem_raw)
+                             - __float_as_uint(kTabMagic) * BondsEntry<kObs>::bytes;
     __syncthreads();
 
     double beta = a.beta;
@@ -195,8 +240,8 @@ k_bonds(const SweepArgs a)
     bcx.phi = a.phi;
     bcx.beta = beta;
     bcx.m2b = (float)(-2.0 * beta * 1.4426950408889634);
+    bcx.delta = filter_delta(beta);
     bcx.fallback_counter = &a.ctl->fallback_count;
-    const double cphi = a.cphi, sphi = a.sphi;
 
     double aMx = 0, aMy = 0, aCx = 0, aSx = 0, aCy = 0, aSy = 0;
     double aF[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // kFourier: Fx[0..3], Fy[0..3]
@@ -214,11 +259,11 @@ k_bonds(const SweepArgs a)
             uint32_t xh = sx * TW + TW;
             if (xh >= L) xh = 0;
             const float th = __ldg(a.theta + (size_t)(y0 + lane) * L + xh);
-            double s, c;
-            sincos_tab(th, tab, s, c);
-            h_c[warp][lane] = c;
-            h_s[warp][lane] = s;
-            h_g[warp][lane] = __double2float_rn(__fma_rn(c, cphi, s * sphi));
+            double s = 0, c = 0;
+            float g = 0;
+            site_eval<kBonds, kObs>(th, tab_adj, g, c, s);
+            if constexpr (kObs) { h_c[warp][lane] = c; h_s[warp][lane] = s; }
+            if constexpr (kBonds) h_g[warp][lane] = g;
             if constexpr (kFourier) {
                 double sk, ck;
                 sincospi(2.0 * (double)(y0 + lane) / (double)L, &sk, &ck);
@@ -230,39 +275,40 @@ k_bonds(const SweepArgs a)
 #pragma unroll
         for (int v = 0; v < VEC; ++v) { colC[v] = 0.0; colS[v] = 0.0; }
 
-        // two register sets (A, B) alternate as "row being finished" and "row below": no copies
+        // two register sets (A, B) alternate as "row being finished" and "row below": no copies.  The raw
+        // angles of rows r+1 and r+2 are in flight while row r is evaluated (a set is reloaded as soon as
+        // its angles are split)
         float tA[VEC], tB[VEC], gA[VEC], gB[VEC];
         double cA[VEC], sA[VEC], cB[VEC], sB[VEC];
-        load_vec<VEC, true>(a.theta + (size_t)y0 * L + xl, tA);
-        {
-            uint32_t y1 = y0 + 1;
-            if (y1 >= L) y1 -= L;
-            load_vec<VEC, true>(a.theta + (size_t)y1 * L + xl, tB);
-        }
+        auto row_ptr = [&](uint32_t r) {
+            uint32_t y = y0 + r;
+            if (y >= L) y -= L;
+            return a.theta + (size_t)y * L + xl;
+        };
+        load_vec<VEC, true>(row_ptr(0), tA);
+        load_vec<VEC, true>(row_ptr(1), tB);
 #pragma unroll
-        for (int v = 0; v < VEC; ++v) {
-            sincos_tab(tA[v], tab, sA[v], cA[v]);
-            gA[v] = __double2float_rn(__fma_rn(cA[v], cphi, sA[v] * sphi));
-        }
+        for (int v = 0; v < VEC; ++v) site_eval<kBonds, kObs>(tA[v], tab_adj, gA[v], cA[v], sA[v]);
+        if (RS >= 2) load_vec<VEC, true>(row_ptr(2), tA);
         // finishes row r-1 (evaluated, in pc/ps/pg): its x bonds, and its y bonds with row r, whose
-        // raw angles are in ct and whose (cos, sin, sigma) land in c/s/g; pt is free for the prefetch
-        auto step = [&](int r, float (&pt)[VEC], const double (&pc)[VEC], const double (&ps)[VEC], const float (&pg)[VEC],
-                        const float (&ct)[VEC], double (&c)[VEC], double (&s)[VEC], float (&g)[VEC]) {
-            if (r < RS) {                                   // prefetch row r+1
-                uint32_t y2 = y0 + r + 1;
-                if (y2 >= L) y2 -= L;
-                load_vec<VEC, true>(a.theta + (size_t)y2 * L + xl, pt);
-            }
+        // raw angles are in ct and whose (cos, sin, sigma) land in c/s/g; then ct is reloaded with row r+2
+        auto step = [&](int r, const double (&pc)[VEC], const double (&ps)[VEC], const float (&pg)[VEC],
+                        float (&ct)[VEC], double (&c)[VEC], double (&s)[VEC], float (&g)[VEC]) {
 #pragma unroll
-            for (int v = 0; v < VEC; ++v) {
-                sincos_tab(ct[v], tab, s[v], c[v]);
-                g[v] = __double2float_rn(__fma_rn(c[v], cphi, s[v] * sphi));
-            }
+            for (int v = 0; v < VEC; ++v) site_eval<kBonds, kObs>(ct[v], tab_adj, g[v], c[v], s[v]);
+            if (r + 2 <= RS) load_vec<VEC, true>(row_ptr(r + 2), ct);
             const uint32_t gy = y0 + r - 1;                 // global row being finished
-            double cn = __shfl_down_sync(0xffffffffu, pc[0], 1);
-            double sn = __shfl_down_sync(0xffffffffu, ps[0], 1);
-            float gn = __shfl_down_sync(0xffffffffu, pg[0], 1);
-            if (lane == 31) { cn = h_c[warp][r - 1]; sn = h_s[warp][r - 1]; gn = h_g[warp][r - 1]; }
+            double cn = 0, sn = 0;
+            float gn = 0;
+            if constexpr (kObs) {
+                cn = __shfl_down_sync(0xffffffffu, pc[0], 1);
+                sn = __shfl_down_sync(0xffffffffu, ps[0], 1);
+                if (lane == 31) { cn = h_c[warp][r - 1]; sn = h_s[warp][r - 1]; }
+            }
+            if constexpr (kBonds) {
+                gn = __shfl_down_sync(0xffffffffu, pg[0], 1);
+                if (lane == 31) gn = h_g[warp][r - 1];
+            }
             // leading 16 bits of the 2 VEC uniforms: word j of call A of the quad serves site 4q+j
             // (x: low half, y: high half); the trailing bits (call B) are drawn only on a close call
             uint32_t wa[VEC];
@@ -273,21 +319,23 @@ k_bonds(const SweepArgs a)
                 else { const bool up = (site0 & 2u) != 0; wa[0] = up ? w.z : w.x; wa[1] = up ? w.w : w.y; }
             }
             uint32_t xn = 0, yn = 0;
-            float dx[VEC], dy[VEC], dmin = 1.0f;
+            float dx[VEC], dy[VEC], dmin = 3.0e38f;
 #pragma unroll
             for (int v = VEC - 1; v >= 0; --v) {
-                const double c2 = (v + 1 < VEC) ? pc[(v + 1) % VEC] : cn;
-                const double s2 = (v + 1 < VEC) ? ps[(v + 1) % VEC] : sn;
-                if constexpr (kFourier) { colC[v] += pc[v]; colS[v] += ps[v]; }
-                else { aMx += pc[v]; aMy += ps[v]; }
-                aCx = __fma_rn(pc[v], c2, aCx);
-                aCx = __fma_rn(ps[v], s2, aCx);
-                aSx = __fma_rn(ps[v], c2, aSx);
-                aSx = __fma_rn(-pc[v], s2, aSx);
-                aCy = __fma_rn(pc[v], c[v], aCy);
-                aCy = __fma_rn(ps[v], s[v], aCy);
-                aSy = __fma_rn(ps[v], c[v], aSy);
-                aSy = __fma_rn(-pc[v], s[v], aSy);
+                if constexpr (kObs) {
+                    const double c2 = (v + 1 < VEC) ? pc[(v + 1) % VEC] : cn;
+                    const double s2 = (v + 1 < VEC) ? ps[(v + 1) % VEC] : sn;
+                    if constexpr (kFourier) { colC[v] += pc[v]; colS[v] += ps[v]; }
+                    else { aMx += pc[v]; aMy += ps[v]; }
+                    aCx = __fma_rn(pc[v], c2, aCx);
+                    aCx = __fma_rn(ps[v], s2, aCx);
+                    aSx = __fma_rn(ps[v], c2, aSx);
+                    aSx = __fma_rn(-pc[v], s2, aSx);
+                    aCy = __fma_rn(pc[v], c[v], aCy);
+                    aCy = __fma_rn(ps[v], s[v], aCy);
+                    aSy = __fma_rn(ps[v], c[v], aSy);
+                    aSy = __fma_rn(-pc[v], s[v], aSy);
+                }
                 if constexpr (kBonds) {
                     const float g2 = (v + 1 < VEC) ? pg[(v + 1) % VEC] : gn;
                     const float gs = pg[v] * bcx.m2b;
@@ -307,19 +355,19 @@ k_bonds(const SweepArgs a)
                 aF[6] = __fma_rn(rs, ky.x, aF[6]); aF[7] = __fma_rn(rs, ky.y, aF[7]);
             }
             if constexpr (kBonds) {
-                if (dmin <= kFilterDelta) {              // rare: some decision of this lane is too close to call
+                if (!(dmin > bcx.delta)) {               // rare: some decision of this lane is too close to call (or NaN)
                     const U4 w = philox4x32_10_rk((uint32_t)(site0 >> 2), (uint32_t)(site0 >> 34), a.t, TAG_BOND_LO, a.rk);
                     uint32_t wb[VEC];
                     if constexpr (VEC == 4) { wb[0] = w.x; wb[1] = w.y; wb[2] = w.z; wb[3] = w.w; }
                     else { const bool up = (site0 & 2u) != 0; wb[0] = up ? w.z : w.x; wb[1] = up ? w.w : w.y; }
 #pragma unroll
                     for (int v = 0; v < VEC; ++v) {
-                        if (fabsf(dx[v]) <= kFilterDelta) {
+                        if (!(fabsf(dx[v]) > bcx.delta)) {
                             const uint32_t wx = (wa[v] << 16) | (wb[v] & 0xffffu);
                             xn &= ~(1u << v);
                             if (bond_exact_at(a.theta, L, gy, xl + v, 0, bcx.phi, bcx.beta, wx, bcx.fallback_counter)) xn |= 1u << v;
                         }
-                        if (fabsf(dy[v]) <= kFilterDelta) {
+                        if (!(fabsf(dy[v]) > bcx.delta)) {
                             const uint32_t wy = (wa[v] & 0xffff0000u) | (wb[v] >> 16);
                             yn &= ~(1u << v);
                             if (bond_exact_at(a.theta, L, gy, xl + v, 1, bcx.phi, bcx.beta, wy, bcx.fallback_counter)) yn |= 1u << v;
@@ -341,8 +389,8 @@ k_bonds(const SweepArgs a)
         static_assert(RS % 2 == 0, "the row loop is unrolled by two");
 #pragma unroll 1
         for (int r = 1; r <= RS; r += 2) {
-            step(r, tA, cA, sA, gA, tB, cB, sB, gB);
-            step(r + 1, tB, cB, sB, gB, tA, cA, sA, gA);
+            step(r, cA, sA, gA, tB, cB, sB, gB);
+            step(r + 1, cB, sB, gB, tA, cA, sA, gA);
         }
         if constexpr (kFourier) {
             double sk, ck;
@@ -366,12 +414,16 @@ k_bonds(const SweepArgs a)
 #pragma unroll
         for (int k = 0; k < 8; ++k) acc[6 + k] = aF[k];
     }
+    if constexpr (kObs) {
 #pragma unroll
-    for (int k = 0; k < NS; ++k) acc[k] = warp_sum(acc[k]);
+        for (int k = 0; k < NS; ++k) acc[k] = warp_sum(acc[k]);
+    }
     unsigned long long cbx = warp_sum_u64(nbx), cby = warp_sum_u64(nby);
     if (lane == 0) {
+        if constexpr (kObs) {
 #pragma unroll
-        for (int k = 0; k < NS; ++k) red[warp][k] = acc[k];
+            for (int k = 0; k < NS; ++k) red[warp][k] = acc[k];
+        }
         redc[warp][0] = cbx; redc[warp][1] = cby;
     }
     __syncthreads();
@@ -380,11 +432,11 @@ k_bonds(const SweepArgs a)
         for (int k = 0; k < NS; ++k) tot[k] = 0.0;
         unsigned long long c0 = 0, c1 = 0;
         for (int w = 0; w < NW; ++w) {
-            for (int k = 0; k < NS; ++k) tot[k] += red[w][k];
+            if constexpr (kObs) for (int k = 0; k < NS; ++k) tot[k] += red[w][k];
             c0 += redc[w][0]; c1 += redc[w][1];
         }
         double *p = a.partials + (size_t)blockIdx.x * kPartialStride;
-        for (int k = 0; k < NS; ++k) p[k] = tot[k];
+        if constexpr (kObs) for (int k = 0; k < NS; ++k) p[k] = tot[k];
         p[14] = __longlong_as_double((long long)c0);
         p[15] = __longlong_as_double((long long)c1);
         __threadfence();
@@ -401,15 +453,15 @@ k_bonds(const SweepArgs a)
         unsigned long long c0 = 0, c1 = 0;
         for (uint32_t b = threadIdx.x; b < gridDim.x; b += blockDim.x) {
             const double *p = a.partials + (size_t)b * kPartialStride;
-            for (int k = 0; k < NS; ++k) acc[k] += __ldcg(p + k);
+            if constexpr (kObs) for (int k = 0; k < NS; ++k) acc[k] += __ldcg(p + k);
             c0 += (unsigned long long)__double_as_longlong(__ldcg(p + 14));
             c1 += (unsigned long long)__double_as_longlong(__ldcg(p + 15));
         }
-        for (int k = 0; k < NS; ++k) acc[k] = warp_sum(acc[k]);
+        if constexpr (kObs) for (int k = 0; k < NS; ++k) acc[k] = warp_sum(acc[k]);
         c0 = warp_sum_u64(c0); c1 = warp_sum_u64(c1);
         __syncthreads();
         if (lane == 0) {
-            for (int k = 0; k < NS; ++k) red[warp][k] = acc[k];
+            if constexpr (kObs) for (int k = 0; k < NS; ++k) red[warp][k] = acc[k];
             redc[warp][0] = c0; redc[warp][1] = c1;
         }
         __syncthreads();
@@ -418,10 +470,19 @@ k_bonds(const SweepArgs a)
             for (int k = 0; k < NS; ++k) tot[k] = 0.0;
             unsigned long long b0 = 0, b1 = 0;
             for (int w = 0; w < NW; ++w) {
-                for (int k = 0; k < NS; ++k) tot[k] += red[w][k];
+                if constexpr (kObs) for (int k = 0; k < NS; ++k) tot[k] += red[w][k];
                 b0 += redc[w][0]; b1 += redc[w][1];
             }
+            // sums that are linear in (cos, sin)(theta - phi): back to the lattice frame,
+            // cos theta = c cos phi - s sin phi, sin theta = s cos phi + c sin phi
+            auto unrotate = [&](double &vc, double &vs) {
+                const double rc = __fma_rn(vc, cphi, -(vs * sphi)), rs = __fma_rn(vs, cphi, vc * sphi);
+                vc = rc; vs = rs;
+            };
+            if constexpr (kObs) unrotate(tot[0], tot[1]);
             if constexpr (kFourier) {
+                unrotate(tot[6], tot[8]); unrotate(tot[7], tot[9]);       // Fx = (c cos kx, c sin kx, s cos kx, s sin kx)
+                unrotate(tot[10], tot[12]); unrotate(tot[11], tot[13]);
                 if (a.obs_fill) {
                     xy_fourier *f = a.fring + (a.t % a.ring_cap);   // record of T = t (the incoming state)
                     f->sweep = (uint64_t)a.t;
@@ -429,12 +490,14 @@ k_bonds(const SweepArgs a)
                 }
             }
             const double N = (double)L * (double)L;
-            if (a.obs_fill) {
-                xy_obs *o = a.ring + (a.t % a.ring_cap);         // record of T = t (the incoming state)
-                o->Mx = tot[0]; o->My = tot[1]; o->Cx = tot[2]; o->Sx = tot[3]; o->Cy = tot[4]; o->Sy = tot[5];
-                o->E = -(tot[2] + tot[4]);
+            if constexpr (kObs) {
+                if (a.obs_fill) {
+                    xy_obs *o = a.ring + (a.t % a.ring_cap);         // record of T = t (the incoming state)
+                    o->Mx = tot[0]; o->My = tot[1]; o->Cx = tot[2]; o->Sx = tot[3]; o->Cy = tot[4]; o->Sy = tot[5];
+                    o->E = -(tot[2] + tot[4]);
+                }
+                if (a.feed_pcc) pcc_feed(a.ctl, N, tot[2], tot[3], tot[4], tot[5]);
             }
-            if (a.feed_pcc) pcc_feed(a.ctl, N, tot[2], tot[3], tot[4], tot[5]);
             if constexpr (kBonds) {
                 xy_obs *o = a.ring + ((a.t + 1u) % a.ring_cap);  // record of T = t+1, completed later
                 o->sweep = (uint64_t)a.t + 1u;
@@ -913,6 +976,43 @@ __global__ void k_flatten(LabelT *labels, uint64_t N)
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (uint64_t)gridDim.x * blockDim.x) {
         const LabelT r = gfind<LabelT>(labels, (LabelT)i);
         labels[i] = r;
+    }
+}
+
+// Whole-lattice invariants of a flattened labeling (xy_debug_check_labels).  out[0]: label[i] > i;
+// out[1]: label[label[i]] != label[i]; out[2] / out[3]: an active x / y bond joins unequal labels
+// (periodic wrap included); out[4]: number of roots (label[i] == i).  A labeling with all four
+// violation counts zero names every cluster by one of its sites, is constant on clusters, and no
+// label is above its site's index.
+template <typename LabelT>
+__global__ void k_check_labels(const LabelT *labels, const uint8_t *bonds, uint32_t L, unsigned long long *out)
+{
+    const uint64_t N = (uint64_t)L * L;
+    unsigned long long v0 = 0, v1 = 0, v2 = 0, v3 = 0, v4 = 0;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (uint64_t)gridDim.x * blockDim.x) {
+        const LabelT l = labels[i];
+        if ((uint64_t)l > i) { ++v0; continue; }
+        if (labels[l] != l) ++v1;
+        if ((uint64_t)l == i) ++v4;
+        const uint32_t b = bonds[i >> 2];
+        const uint32_t j = (uint32_t)(i & 3u);
+        const uint32_t x = (uint32_t)(i % L);
+        if ((b >> j) & 1u) {
+            const uint64_t r = (x + 1 == L) ? i + 1 - L : i + 1;
+            if (labels[r] != l) ++v2;
+        }
+        if ((b >> (4 + j)) & 1u) {
+            const uint64_t d = (i + L >= N) ? i + L - N : i + L;
+            if (labels[d] != l) ++v3;
+        }
+    }
+    v0 = warp_sum_u64(v0); v1 = warp_sum_u64(v1); v2 = warp_sum_u64(v2); v3 = warp_sum_u64(v3); v4 = warp_sum_u64(v4);
+    if ((threadIdx.x & 31) == 0) {
+        if (v0) atomicAdd(out + 0, v0);
+        if (v1) atomicAdd(out + 1, v1);
+        if (v2) atomicAdd(out + 2, v2);
+        if (v3) atomicAdd(out + 3, v3);
+        if (v4) atomicAdd(out + 4, v4);
     }
 }
 
