@@ -219,6 +219,8 @@ def main():
     ap.add_argument("--fourier", action="store_true",
                     help="also reduce the structure-factor sums of every sweep (xi_2nd; XY_FLAG_FOURIER)")
     ap.add_argument("--beta", type=float, default=None, help="override the workload's beta (sensitivity runs)")
+    ap.add_argument("--obs", default="all", choices=["all", "none"],
+                    help="none: time the sweeps with the observable sums switched off (xy_set_obs_mode); not the headline")
     ap.add_argument("--e2e-steps", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -251,6 +253,8 @@ def main():
     K, W = args.steps, max(args.warmup, 0)
 
     st = xy.XYState(L, replica_seed(seed, rank), xy_inputs.INIT_CODE[init], flags=flags)
+    if args.obs == "none":
+        st.set_obs_mode(xy.OBS_NONE)
     if therm:
         st.sw_sweeps(beta, therm)
     st.sw_sweeps(beta, W)

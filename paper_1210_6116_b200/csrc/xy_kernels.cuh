@@ -201,6 +201,48 @@ __device__ __forceinline__ void site_eval(float theta, uint32_t tab_adj, float &
     }
 }
 
+// Cold path of k_bonds: some decision of this lane's VEC sites in row gy was too close for the filter.
+// Everything is recomputed from the values the hot loop still holds (sigma of the row, of the row below and
+// of the right neighbour), so the hot loop keeps no per-bond state alive for it: call A again, call B for
+// the trailing bits, the same filter arithmetic (bit-identical d), and the fp64 definition for every bond
+// with |d| <= delta.  bits = xn | yn << 8 as the filter decided them; returns the corrected bits.
+template <int VEC> struct RowSigma { float pg[VEC], g[VEC], gn; };
+
+template <int VEC>
+__device__ __noinline__ uint32_t bonds_fix(const float *theta, uint32_t L, uint32_t seed_lo, uint32_t seed_hi, uint32_t t,
+                                           BondCtx bcx, uint64_t quad, uint32_t gy, uint32_t xl, RowSigma<VEC> rs, uint32_t bits)
+{
+    const U4 wA = rng(seed_lo, seed_hi, quad, t, TAG_BOND);
+    const U4 wB = rng(seed_lo, seed_hi, quad, t, TAG_BOND_LO);
+    uint32_t wa[VEC], wb[VEC];
+    if constexpr (VEC == 4) {
+        wa[0] = wA.x; wa[1] = wA.y; wa[2] = wA.z; wa[3] = wA.w;
+        wb[0] = wB.x; wb[1] = wB.y; wb[2] = wB.z; wb[3] = wB.w;
+    } else {
+        const bool up = (xl & 2u) != 0;
+        wa[0] = up ? wA.z : wA.x; wa[1] = up ? wA.w : wA.y;
+        wb[0] = up ? wB.z : wB.x; wb[1] = up ? wB.w : wB.y;
+    }
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) {
+        const float g2 = (v + 1 < VEC) ? rs.pg[(v + 1) % VEC] : rs.gn;
+        const float gs = rs.pg[v] * bcx.m2b;
+        const float dx = bond_filter(gs, g2, wa[v] << 7);
+        const float dy = bond_filter(gs, rs.g[v], wa[v] >> 9);
+        if (!(fabsf(dx) > bcx.delta)) {
+            const uint32_t wx = (wa[v] << 16) | (wb[v] & 0xffffu);
+            bits &= ~(1u << v);
+            if (bond_exact_at(theta, L, gy, xl + v, 0, bcx.phi, bcx.beta, wx, bcx.fallback_counter)) bits |= 1u << v;
+        }
+        if (!(fabsf(dy) > bcx.delta)) {
+            const uint32_t wy = (wa[v] & 0xffff0000u) | (wb[v] >> 16);
+            bits &= ~(0x100u << v);
+            if (bond_exact_at(theta, L, gy, xl + v, 1, bcx.phi, bcx.beta, wy, bcx.fallback_counter)) bits |= 0x100u << v;
+        }
+    }
+    return bits;
+}
+
 template <int VEC, int RS, bool kBonds, bool kObs, bool kFourier>
 __global__ void __launch_bounds__(kBondsWarps * 32, kObs ? 1 : 2)
 k_bonds(const SweepArgs a)
@@ -234,14 +276,16 @@ k_bonds(const SweepArgs a)
                              - __float_as_uint(kTabMagic) * BondsEntry<kObs>::bytes;
     __syncthreads();
 
-    double beta = a.beta;
-    if (a.beta_from_ctl) beta = *reinterpret_cast<const volatile double *>(&a.ctl->beta);
-    BondCtx bcx;
-    bcx.phi = a.phi;
-    bcx.beta = beta;
-    bcx.m2b = (float)(-2.0 * beta * 1.4426950408889634);
-    bcx.delta = filter_delta(beta);
-    bcx.fallback_counter = &a.ctl->fallback_count;
+    // beta: a kernel argument, or (PCC) the controller's; only its two fp32 derivatives stay in registers
+    auto load_beta = [&]() {
+        return a.beta_from_ctl ? *reinterpret_cast<const volatile double *>(&a.ctl->beta) : a.beta;
+    };
+    float m2b, delta;
+    {
+        const double beta = load_beta();
+        m2b = (float)(-2.0 * beta * 1.4426950408889634);
+        delta = filter_delta(beta);
+    }
 
     double aMx = 0, aMy = 0, aCx = 0, aSx = 0, aCy = 0, aSy = 0;
     double aF[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // kFourier: Fx[0..3], Fy[0..3]
@@ -280,23 +324,30 @@ k_bonds(const SweepArgs a)
         // its angles are split)
         float tA[VEC], tB[VEC], gA[VEC], gB[VEC];
         double cA[VEC], sA[VEC], cB[VEC], sB[VEC];
-        auto row_ptr = [&](uint32_t r) {
-            uint32_t y = y0 + r;
-            if (y >= L) y -= L;
-            return a.theta + (size_t)y * L + xl;
-        };
-        load_vec<VEC, true>(row_ptr(0), tA);
-        load_vec<VEC, true>(row_ptr(1), tB);
+        // running addresses (one 64-bit add per row each): quad index of the lane's first site in the row
+        // being finished (Philox counter, bond byte), and the row to load next; only the y-halo row of the
+        // lattice's last strip row wraps
+        uint64_t quad = ((uint64_t)y0 * L + xl) >> 2;
+        const float *nxt = a.theta + (size_t)y0 * L + xl;
+        const float *halo_row = a.theta + (y0 + RS == L ? (size_t)0 : (size_t)(y0 + RS) * L) + xl;
+        load_vec<VEC, true>(nxt, tA);
+        nxt += L;
+        load_vec<VEC, true>(RS == 1 ? halo_row : nxt, tB);
+        nxt += L;
 #pragma unroll
         for (int v = 0; v < VEC; ++v) site_eval<kBonds, kObs>(tA[v], tab_adj, gA[v], cA[v], sA[v]);
-        if (RS >= 2) load_vec<VEC, true>(row_ptr(2), tA);
+        load_vec<VEC, true>(RS == 2 ? halo_row : nxt, tA);
+        nxt += L;
         // finishes row r-1 (evaluated, in pc/ps/pg): its x bonds, and its y bonds with row r, whose
         // raw angles are in ct and whose (cos, sin, sigma) land in c/s/g; then ct is reloaded with row r+2
         auto step = [&](int r, const double (&pc)[VEC], const double (&ps)[VEC], const float (&pg)[VEC],
                         float (&ct)[VEC], double (&c)[VEC], double (&s)[VEC], float (&g)[VEC]) {
 #pragma unroll
             for (int v = 0; v < VEC; ++v) site_eval<kBonds, kObs>(ct[v], tab_adj, g[v], c[v], s[v]);
-            if (r + 2 <= RS) load_vec<VEC, true>(row_ptr(r + 2), ct);
+            if (r + 2 <= RS) {
+                load_vec<VEC, true>(r + 2 == RS ? halo_row : nxt, ct);
+                nxt += L;
+            }
             const uint32_t gy = y0 + r - 1;                 // global row being finished
             double cn = 0, sn = 0;
             float gn = 0;
@@ -312,14 +363,13 @@ k_bonds(const SweepArgs a)
             // leading 16 bits of the 2 VEC uniforms: word j of call A of the quad serves site 4q+j
             // (x: low half, y: high half); the trailing bits (call B) are drawn only on a close call
             uint32_t wa[VEC];
-            const uint64_t site0 = (uint64_t)gy * L + xl;
             if constexpr (kBonds) {
-                const U4 w = philox4x32_10_rk((uint32_t)(site0 >> 2), (uint32_t)(site0 >> 34), a.t, TAG_BOND, a.rk);
+                const U4 w = philox4x32_10_rk((uint32_t)quad, (uint32_t)(quad >> 32), a.t, TAG_BOND, a.rk);
                 if constexpr (VEC == 4) { wa[0] = w.x; wa[1] = w.y; wa[2] = w.z; wa[3] = w.w; }
-                else { const bool up = (site0 & 2u) != 0; wa[0] = up ? w.z : w.x; wa[1] = up ? w.w : w.y; }
+                else { const bool up = (xl & 2u) != 0; wa[0] = up ? w.z : w.x; wa[1] = up ? w.w : w.y; }
             }
             uint32_t xn = 0, yn = 0;
-            float dx[VEC], dy[VEC], dmin = 3.0e38f;
+            float dmin = 3.0e38f;
 #pragma unroll
             for (int v = VEC - 1; v >= 0; --v) {
                 if constexpr (kObs) {
@@ -338,12 +388,12 @@ k_bonds(const SweepArgs a)
                 }
                 if constexpr (kBonds) {
                     const float g2 = (v + 1 < VEC) ? pg[(v + 1) % VEC] : gn;
-                    const float gs = pg[v] * bcx.m2b;
-                    dx[v] = bond_filter(gs, g2, wa[v] << 7);
-                    dy[v] = bond_filter(gs, g[v], wa[v] >> 9);
-                    dmin = fminf(dmin, fminf(fabsf(dx[v]), fabsf(dy[v])));
-                    xn = __funnelshift_l(__float_as_uint(dx[v]), xn, 1);      // (xn << 1) | sign(dx): active iff d < 0
-                    yn = __funnelshift_l(__float_as_uint(dy[v]), yn, 1);
+                    const float gs = pg[v] * m2b;
+                    const float dx = bond_filter(gs, g2, wa[v] << 7);
+                    const float dy = bond_filter(gs, g[v], wa[v] >> 9);
+                    dmin = fminf(dmin, fminf(fabsf(dx), fabsf(dy)));
+                    xn = __funnelshift_l(__float_as_uint(dx), xn, 1);         // (xn << 1) | sign(dx): active iff d < 0
+                    yn = __funnelshift_l(__float_as_uint(dy), yn, 1);
                 }
             }
             if constexpr (kFourier) {
@@ -355,36 +405,33 @@ k_bonds(const SweepArgs a)
                 aF[6] = __fma_rn(rs, ky.x, aF[6]); aF[7] = __fma_rn(rs, ky.y, aF[7]);
             }
             if constexpr (kBonds) {
-                if (!(dmin > bcx.delta)) {               // rare: some decision of this lane is too close to call (or NaN)
-                    const U4 w = philox4x32_10_rk((uint32_t)(site0 >> 2), (uint32_t)(site0 >> 34), a.t, TAG_BOND_LO, a.rk);
-                    uint32_t wb[VEC];
-                    if constexpr (VEC == 4) { wb[0] = w.x; wb[1] = w.y; wb[2] = w.z; wb[3] = w.w; }
-                    else { const bool up = (site0 & 2u) != 0; wb[0] = up ? w.z : w.x; wb[1] = up ? w.w : w.y; }
+                if (!(dmin > delta)) {                   // rare: some decision of this lane is too close to call (or NaN)
+                    BondCtx bcx;
+                    bcx.phi = a.phi;
+                    bcx.beta = load_beta();
+                    bcx.m2b = m2b;
+                    bcx.delta = delta;
+                    bcx.fallback_counter = &a.ctl->fallback_count;
+                    RowSigma<VEC> rsg;
 #pragma unroll
-                    for (int v = 0; v < VEC; ++v) {
-                        if (!(fabsf(dx[v]) > bcx.delta)) {
-                            const uint32_t wx = (wa[v] << 16) | (wb[v] & 0xffffu);
-                            xn &= ~(1u << v);
-                            if (bond_exact_at(a.theta, L, gy, xl + v, 0, bcx.phi, bcx.beta, wx, bcx.fallback_counter)) xn |= 1u << v;
-                        }
-                        if (!(fabsf(dy[v]) > bcx.delta)) {
-                            const uint32_t wy = (wa[v] & 0xffff0000u) | (wb[v] >> 16);
-                            yn &= ~(1u << v);
-                            if (bond_exact_at(a.theta, L, gy, xl + v, 1, bcx.phi, bcx.beta, wy, bcx.fallback_counter)) yn |= 1u << v;
-                        }
-                    }
+                    for (int v = 0; v < VEC; ++v) { rsg.pg[v] = pg[v]; rsg.g[v] = g[v]; }
+                    rsg.gn = gn;
+                    const uint32_t fixed = bonds_fix<VEC>(a.theta, L, a.seed_lo, a.seed_hi, a.t, bcx, quad, gy, xl, rsg, xn | (yn << 8));
+                    xn = fixed & 0xffu;
+                    yn = fixed >> 8;
                 }
                 nbx += __popc(xn);
                 nby += __popc(yn);
                 if constexpr (VEC == 4) {
-                    a.bonds[((size_t)gy * L + xl) >> 2] = (uint8_t)(xn | (yn << 4));
+                    a.bonds[quad] = (uint8_t)(xn | (yn << 4));
                 } else {
                     // two lanes share a byte: even lane holds sites 4k,4k+1; odd lane 4k+2,4k+3
                     const uint32_t mine = xn | (yn << 4);
                     const uint32_t other = __shfl_xor_sync(0xffffffffu, mine, 1);
-                    if ((lane & 1) == 0) a.bonds[((size_t)gy * L + xl) >> 2] = (uint8_t)(mine | (other << 2));
+                    if ((lane & 1) == 0) a.bonds[quad] = (uint8_t)(mine | (other << 2));
                 }
             }
+            quad += L >> 2;
         };
         static_assert(RS % 2 == 0, "the row loop is unrolled by two");
 #pragma unroll 1
@@ -501,7 +548,7 @@ k_bonds(const SweepArgs a)
             if constexpr (kBonds) {
                 xy_obs *o = a.ring + ((a.t + 1u) % a.ring_cap);  // record of T = t+1, completed later
                 o->sweep = (uint64_t)a.t + 1u;
-                o->beta = beta;
+                o->beta = load_beta();
                 const double qnan = __longlong_as_double(0x7ff8000000000000LL);
                 o->E = qnan; o->Mx = qnan; o->My = qnan; o->Cx = qnan; o->Sx = qnan; o->Cy = qnan; o->Sy = qnan;
                 o->n_bonds_x = b0; o->n_bonds_y = b1; o->n_clusters = 0;
