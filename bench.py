@@ -134,6 +134,129 @@ def cpu_oracle_rate(beta, budget_s=20.0, max_sweeps=None):
     return L * L * n / dt, n, dt
 
 
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def cpu_oracle_all_cores(beta, budget_s=15.0):
+    """nproc independent oracle replicas (one per thread, own lattice and seed; ctypes releases the GIL), the way
+    a CPU would parallelise this Monte Carlo: aggregate spin updates/s."""
+    from concurrent.futures import ThreadPoolExecutor
+    from oracle import xy_oracle as xo
+    L = CPU_SAMPLE_L
+    ncores = os.cpu_count() or 1
+    t0 = time.perf_counter()
+    xo.run(xo.init(L, 13, xo.INIT_COLD), L, 13, 0, beta, 1, series=True)
+    per = time.perf_counter() - t0
+    n = max(2, int(budget_s / max(per, 1e-3) / 1.5))       # all cores busy: expect some slowdown per replica
+
+    def replica(r):
+        th = xo.init(L, 100 + r, xo.INIT_COLD)
+        xo.run(th, L, 100 + r, 0, beta, n, series=True)
+
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(max_workers=ncores) as ex:
+        list(ex.map(replica, range(ncores)))
+    dt = time.perf_counter() - t0
+    return ncores * L * L * n / dt, ncores, n, dt
+
+
+def issue_model(workload):
+    """warp instructions per launch of each kernel, from the committed ncu summary (profiles/instr.csv)"""
+    out = {}
+    path = os.path.join(ROOT, "profiles", "instr.csv")
+    if os.path.exists(path):
+        try:
+            for row in open(path).read().split()[1:]:
+                w, kname, n = row.split(",")
+                if w == workload:
+                    out[kname] = float(n)
+        except Exception:
+            return {}
+    return out
+
+
+def timed_leg(xy, torch, L, init, seed, beta, flags=0, therm=0, warm=3, K=20, obs="all", per_sweep=False, check=False):
+    """one extra workload of the `also` block: K sweeps timed with CUDA events after therm + warm untimed sweeps;
+    per_sweep: an event pair around every sweep (time series); check: the device-side label invariants after every
+    timed sweep (outside the event pairs)."""
+    N = L * L
+    lb = 8 if flags & xy.FLAG_LABELS64 else 4
+    tw, th = (128, 32) if L % 128 == 0 else (64, 32)
+    st = xy.XYState(L, seed, xy_inputs.INIT_CODE[init], flags=flags)
+    if obs == "none":
+        st.set_obs_mode(xy.OBS_NONE)
+    if therm + warm:
+        st.sw_sweeps(beta, therm + warm)
+    torch.cuda.synchronize()
+    bad = 0
+    if per_sweep or check:
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * K)]
+        for k in range(K):
+            ev[2 * k].record()
+            st.sw_sweeps(beta, 1)
+            ev[2 * k + 1].record()
+            if check:
+                inv = st.debug_check_labels()
+                bad += inv["label_above_index"] + inv["root_not_fixed"] + inv["x_bond_split"] + inv["y_bond_split"]
+        torch.cuda.synchronize()
+        times = sorted(ev[2 * k].elapsed_time(ev[2 * k + 1]) for k in range(K))
+        ms = sum(times)
+    else:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        st.sw_sweeps(beta, K)
+        e1.record()
+        torch.cuda.synchronize()
+        ms, times = e0.elapsed_time(e1), None
+    o = st.measure()
+    st.destroy()
+    del st
+    torch.cuda.empty_cache()
+    bps = sum(bytes_model(L, lb, tw, th).values())
+    peak, _ = measured_peaks()
+    out = {"L": L, "init": init, "seed": seed, "beta": beta, "label_bytes": lb, "observables": obs, "untimed_sweeps": therm + warm,
+           "steps": K, "ms_per_step": ms / K, "updates_per_s": N * K / (ms * 1e-3), "bytes_per_site": bps,
+           "sweep_roofline_frac": bps * N * K / (ms * 1e-3) / 1e9 / peak,
+           "bond_density": (o.n_bonds_x + o.n_bonds_y) / (2 * N), "clusters_per_site": o.n_clusters / N}
+    if (4 + lb) * N < 4 * 126e6:
+        out["note"] = "working set comparable to the 126 MB L2: not an HBM measurement"
+    if times:
+        out["per_sweep_ms"] = {"min": times[0], "median": times[len(times) // 2], "max": times[-1]}
+    if check:
+        out["label_invariant_violations"] = int(bad)
+    return out
+
+
+def labeling_only(xy, torch, L, kinds=("all_on", "h_stripes", "serpentine"), reps=3):
+    """the labeling kernels alone (k_label + k_merge, xy_label_bonds) on adversarial bond sets: ms per launch"""
+    st = xy.XYState(L, 1, xy.INIT_COLD)
+    st.debug_kernel_timing(True)
+    out = {}
+    for kind in kinds:
+        b = xy_inputs.pattern_bonds(L, kind)
+        st.label_bonds(b)
+        st.get_kernel_times()
+        for _ in range(reps):
+            st.label_bonds(b)
+        kt = st.get_kernel_times()
+        inv = st.debug_check_labels()
+        out[kind] = {"k_label_ms": kt["k_label"]["ms"] / reps, "k_merge_ms": kt["k_merge"]["ms"] / reps,
+                     "clusters": inv["n_roots"],
+                     "violations": inv["label_above_index"] + inv["root_not_fixed"] + inv["x_bond_split"] + inv["y_bond_split"]}
+        del b
+    st.debug_kernel_timing(False)
+    st.destroy()
+    torch.cuda.empty_cache()
+    return out
+
+
 def run_reference(args, rank, world):
     """--impl reference: the CPU oracle timed on the host cores (rank 0 only)."""
     if rank != 0:
@@ -224,6 +347,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-also", action="store_true",
+                    help="skip the `also` block (configs 3 and 5, masked-observable variants, adversarial labeling)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -304,9 +429,23 @@ def main():
                     traffic = int(nbytes)
         except Exception:
             traffic = None
+    # issue-rate roofline beside the HBM one: warp instructions per launch (ncu, profiles/instr.csv) over the
+    # time the kernel took, against one warp instruction per cycle and scheduler
+    imodel = issue_model(args.workload)
+    sm_mhz = clocks.get("sm_mhz") or 1965.0
+    sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    issue_peak = sms * 4 * sm_mhz * 1e6
+    for name in kern:
+        if name in imodel and kern[name]["avg_ms"] > 0:
+            kern[name]["warp_instr_per_launch"] = imodel[name]
+            kern[name]["issue_frac"] = imodel[name] / (kern[name]["avg_ms"] * 1e-3) / issue_peak
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["achieved_gbs"], "peak": peak,
                 "unit": "GB/s", "frac": kern[dom]["frac"], "traffic": traffic, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": model[dom] * N}
+                "algorithmic_bytes_per_launch": model[dom] * N,
+                "limited_by": "instruction issue / shared-memory wavefronts, not DRAM (profiles/r2_cfg4.md): the HBM "
+                              "fraction is this kernel's distance from its byte floor",
+                "issue": {"warp_instr_per_launch": imodel.get(dom), "peak_warp_instr_per_s": issue_peak,
+                          "frac": kern[dom].get("issue_frac")}}
 
     # ---- e2e: host buffers through the C-ABI every step ----
     e2e = None
@@ -331,10 +470,37 @@ def main():
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        rate, n, dt = cpu_oracle_rate(beta)
+        rate, n, dt = cpu_oracle_rate(beta, budget_s=12.0)
+        arate, ncores, an, adt = cpu_oracle_all_cores(beta, budget_s=12.0)
         cpu = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": f"{n} oracle sweeps of a {CPU_SAMPLE_L}x{CPU_SAMPLE_L} cold-start lattice at beta={beta} "
-                         f"({dt:.1f} s, single thread; 1/{(L // CPU_SAMPLE_L) ** 2 if L >= CPU_SAMPLE_L else 1} of the workload's sites)"}
+                         f"({dt:.1f} s, single thread; 1/{(L // CPU_SAMPLE_L) ** 2 if L >= CPU_SAMPLE_L else 1} of the workload's sites)",
+               "all_cores": {"value": arate, "unit": UNIT, "cores": ncores, "cpu": cpu_model(),
+                             "sample": f"{ncores} independent replicas (one thread each, own seed) x {an} oracle sweeps of a "
+                                       f"{CPU_SAMPLE_L}x{CPU_SAMPLE_L} lattice, {adt:.1f} s"}}
+
+    # ---- also: the ends of the metric's L range, the masked-observable variants, adversarial labeling ----
+    also = None
+    if rank == 0 and world == 1 and not args.no_also and args.workload == "cfg4":
+        st.destroy()
+        st = None
+        torch.cuda.empty_cache()
+        c3, c5 = WORKLOADS["cfg3"], WORKLOADS["cfg5"]
+        also = {
+            "cfg4_observables_off": timed_leg(xy, torch, L, init, seed, beta, therm=therm, warm=W, K=min(K, 50), obs="none"),
+            "cfg3_L4096": timed_leg(xy, torch, c3[1], c3[2], c3[3], c3[4], therm=c3[5], warm=W, K=200),
+            "cfg5_L65536_i64_labels": timed_leg(xy, torch, c5[1], c5[2], c5[3], c5[4], flags=xy.FLAG_LABELS64, warm=0, K=200,
+                                                per_sweep=True, check=True),
+            "cfg5_L65536_u32_labels": timed_leg(xy, torch, c5[1], c5[2], c5[3], c5[4], warm=0, K=200, per_sweep=True),
+            "cfg5_L65536_i64_cold_100_warmup": timed_leg(xy, torch, c5[1], "cold", c5[3], c5[4], flags=xy.FLAG_LABELS64,
+                                                         warm=100, K=20, per_sweep=True),
+            "cfg5_L65536_i64_observables_off": timed_leg(xy, torch, c5[1], c5[2], c5[3], c5[4], flags=xy.FLAG_LABELS64,
+                                                         warm=20, K=20, obs="none"),
+            "labeling_only_L16384": labeling_only(xy, torch, 16384),
+            "note": "value / ms_per_step above are config 4 with all six sums on; entries here are labelled variants, "
+                    "never the headline.  cfg5 is timed from the hot start as BASELINE config 5 states (its first "
+                    "sweeps are transient: see per_sweep_ms)",
+        }
 
     if rank == 0:
         line = {
@@ -350,7 +516,7 @@ def main():
                        if (4 + label_bytes) * N > 4 * 126e6 else "working set fits L2: number is NOT an HBM measurement"},
             "clocks": clocks, "gpu_launches": int(launches),
             "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
-            "kernels": kern,
+            "kernels": kern, "also": also,
             "sweep_roofline": {"bytes_per_site": sweep_bytes, "achieved_gbs": sweep_gbs, "frac": sweep_gbs / peak,
                                "floor_bytes_per_site": 8.0 + 2 * label_bytes,
                                "ns_per_site": ms * 1e6 / (K * N)},
@@ -360,7 +526,8 @@ def main():
                             "clusters_per_site": obs.n_clusters / N},
         }
         print(json.dumps(line), flush=True)
-    st.destroy()
+    if st is not None:
+        st.destroy()
     grp.close()
 
 

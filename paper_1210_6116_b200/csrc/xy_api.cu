@@ -915,11 +915,28 @@ int xy_label_bonds(xy_state *s, const uint8_t *host_bonds, size_t n)
         CUDA_TRY(cudaStreamSynchronize(s->stream));
     }
     SweepArgs a = base_args(s);
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    if (s->timing) {
+        if (int rc = timing_flush(s)) return rc;
+        for (auto &e : ev) CUDA_TRY(cudaEventCreate(&e));
+        CUDA_TRY(cudaEventRecord(ev[0], s->stream));
+    }
     s->ker.label(a, s->stream);
+    if (s->timing) CUDA_TRY(cudaEventRecord(ev[1], s->stream));
     s->ker.merge(a, s->stream);
+    if (s->timing) CUDA_TRY(cudaEventRecord(ev[2], s->stream));
     s->launches += 2;
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaStreamSynchronize(s->stream));
+    if (s->timing) {                      // labeling-only timings land in the k_label / k_merge accumulators
+        for (int j = 0; j < 2; ++j) {
+            float ms = 0;
+            CUDA_TRY(cudaEventElapsedTime(&ms, ev[j], ev[j + 1]));
+            s->t_ms[1 + j] += ms;
+            s->t_n[1 + j] += 1;
+        }
+        for (auto &e : ev) cudaEventDestroy(e);
+    }
     s->have_sweep = true;
     s->labels_flat = false;
     return XY_OK;
