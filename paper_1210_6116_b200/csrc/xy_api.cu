@@ -87,7 +87,7 @@ struct KS {
     template <bool kB, bool kO, bool kF>
     static cudaError_t bonds_launch(const SweepArgs &a, int grid, cudaStream_t st)
     {
-        k_bonds<VEC, RS, kB, kO, kF><<<grid, kBondsWarps * 32, k_bonds_smem_bytes<kO>(), st>>>(a);
+        k_bonds<VEC, RS, kB, kO, kF><<<grid, BondsShape<kO>::warps * 32, k_bonds_smem_bytes<kO>(), st>>>(a);
         return cudaGetLastError();
     }
     static cudaError_t bonds(const SweepArgs &a, int what, bool fourier, int grid, cudaStream_t st)
@@ -120,7 +120,7 @@ struct KS {
                                              (int)k_bonds_smem_bytes<kO>());
         if (e != cudaSuccess) return e;
         int n = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_bonds<VEC, RS, kB, kO, kF>, kBondsWarps * 32,
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_bonds<VEC, RS, kB, kO, kF>, BondsShape<kO>::warps * 32,
                                                           k_bonds_smem_bytes<kO>());
         if (occ && (*occ == 0 || n < *occ)) *occ = n;
         return e;
@@ -496,11 +496,12 @@ int xy_create_ex(xy_state **out, uint32_t L, uint64_t seed, int init, uint32_t f
     const uint32_t ntiles = (L / s->ker.tw) * (L / s->ker.th);
     const uint32_t nstrips = (L / s->ker.tw) * (L / s->ker.rs);
     // the variants of k_bonds with observables share ONE grid so that their fixed-order sums agree bitwise
-    const long need = (nstrips + kBondsWarps - 1) / kBondsWarps;
+    long need = (nstrips + BondsShape<true>::warps - 1) / BondsShape<true>::warps;
     long g = (long)sms * bo;
     if (g > need) g = need;
     if (g > (long)kMaxGrid) g = kMaxGrid;
     s->grid_bonds = (int)g;
+    need = (nstrips + BondsShape<false>::warps - 1) / BondsShape<false>::warps;
     g = (long)sms * bn;
     if (g > need) g = need;
     if (g > (long)kMaxGrid) g = kMaxGrid;
