@@ -196,6 +196,12 @@ int xy_debug_philox(const uint32_t *ctr_host, const uint32_t *key_host, uint32_t
 /* Same inputs through NVIDIA cuRAND's curand_Philox4x32_10 device function (independent pin). */
 int xy_debug_curand_philox(const uint32_t *ctr_host, const uint32_t *key_host, uint32_t *out_host, size_t n);
 
+/* Range-check counters of a library built with -DXY_CHECKED (every data-derived index of the kernels is
+ * checked and violations counted: [0] sincos table entry, [1] tile-local parent offset, [2] wave-list site,
+ * [3] label chased in global memory, [4] k_flip queue slot, [5] coin-table index).  *checked_build = 0 and
+ * all zeros from the normal build, which compiles the checks away. */
+int xy_debug_check_counts(uint64_t counts[8], int *checked_build);
+
 const char *xy_last_error(void);
 
 #ifdef __cplusplus

@@ -106,6 +106,7 @@ _SIGS = {
     "xy_get_kernel_times": [_vp, C.POINTER(C.c_double), C.POINTER(C.c_uint64)],
     "xy_get_launch_count": [_vp, C.POINTER(C.c_uint64)],
     "xy_label_bonds": [_vp, _vp, C.c_size_t],
+    "xy_debug_check_counts": [C.POINTER(C.c_uint64), C.POINTER(C.c_int)],
     "xy_debug_philox": [_vp, _vp, _vp, C.c_size_t],
     "xy_debug_curand_philox": [_vp, _vp, _vp, C.c_size_t],
 }
@@ -291,6 +292,14 @@ def _philox_common(fn, ctr, key):
     out = np.zeros_like(ctr)
     _check(fn(ctr.ctypes.data, key.ctypes.data, out.ctypes.data, ctr.shape[0]))
     return out
+
+
+def debug_check_counts():
+    """(counts[8], checked_build) of the -DXY_CHECKED range checks; all zero from the normal build"""
+    c = (C.c_uint64 * 8)()
+    flag = C.c_int()
+    _check(_lib.xy_debug_check_counts(c, C.byref(flag)))
+    return [int(v) for v in c], bool(flag.value)
 
 
 def debug_philox(ctr, key):

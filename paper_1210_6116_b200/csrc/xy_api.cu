@@ -819,6 +819,22 @@ int xy_get_fourier_series(xy_state *s, xy_fourier *host, uint64_t first, uint64_
     return XY_OK;
 }
 
+int xy_debug_check_counts(uint64_t counts[8], int *checked_build)
+{
+    if (!counts || !checked_build) return fail(XY_ERR_ARG, "NULL argument");
+    for (int k = 0; k < 8; ++k) counts[k] = 0;
+#ifdef XY_CHECKED
+    *checked_build = 1;
+    unsigned long long h[8];
+    CUDA_TRY(cudaDeviceSynchronize());
+    CUDA_TRY(cudaMemcpyFromSymbol(h, g_xy_check_fail, sizeof h));
+    for (int k = 0; k < 8; ++k) counts[k] = h[k];
+#else
+    *checked_build = 0;
+#endif
+    return XY_OK;
+}
+
 int xy_get_fallback_count(xy_state *s, uint64_t *count)
 {
     if (!s || !count) return fail(XY_ERR_ARG, "NULL argument");

@@ -10,6 +10,18 @@ namespace xy {
 constexpr double kTwoPi = 6.283185307179586;   // fl64(2 pi)
 constexpr double kPi    = 3.141592653589793;   // fl64(pi)
 
+// Checked build (-DXY_CHECKED, see profiles/r2_checked_build.md): every index the kernels derive from data
+// (table entry, tile-local parent offset, queue slot, label chased in global memory) is range-checked and
+// violations are counted per site of the check; the normal build compiles the checks away.  This stands in
+// for compute-sanitizer memcheck, which is closed on the pool this was developed on.
+#ifdef XY_CHECKED
+__device__ unsigned long long g_xy_check_fail[8];
+#define XY_CHECK(code, cond) do { if (!(cond)) atomicAdd(&xy::g_xy_check_fail[code], 1ULL); } while (0)
+#else
+#define XY_CHECK(code, cond) do { } while (0)
+#endif
+enum : int { CHK_TABLE = 0, CHK_PARENT = 1, CHK_WLIST = 2, CHK_GLABEL = 3, CHK_QUEUE = 4, CHK_LOC = 5 };
+
 enum : uint32_t { TAG_INIT = 0, TAG_DIR = 1, TAG_BOND = 2, TAG_FLIP = 3, TAG_BOND_LO = 4 };
 
 // ---------------------------------------------------------------------------------------------
@@ -161,7 +173,7 @@ template <typename LabelT>
 __device__ __forceinline__ LabelT gfind(LabelT *lab, LabelT a)
 {
     LabelT r = gload(lab + a);
-    while (r != a) { a = r; r = gload(lab + a); }
+    while (r != a) { XY_CHECK(CHK_GLABEL, r < a); a = r; r = gload(lab + a); }
     return a;
 }
 

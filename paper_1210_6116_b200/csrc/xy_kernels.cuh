@@ -187,6 +187,7 @@ __device__ __forceinline__ void site_eval(float theta, uint32_t tab_adj, float &
     const float h = __fadd_rn(tm, -kTabMagic);
     const float x = __fadd_rn(theta, -h);
     const uint32_t addr = __float_as_uint(tm) * BondsEntry<kObs>::bytes + tab_adj;
+    XY_CHECK(CHK_TABLE, __float_as_uint(tm) - __float_as_uint(kTabMagic) <= (uint32_t)kTabN);
     if constexpr (kObs) {
         double C, S;
         asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(C), "=d"(S) : "r"(addr));
@@ -738,7 +739,10 @@ k_label(const SweepArgs a)
     // it: either way a node of the right component to start the finds from
     unsigned char *pb = reinterpret_cast<unsigned char *>(parent);
     auto unite_at = [&](uint32_t site) {
-        sunion_v(pb, pload(pb, site * 2u), pload(pb, (site + TW) * 2u));
+        XY_CHECK(CHK_WLIST, site + TW < (uint32_t)(TW * TH));
+        const uint32_t ea = pload(pb, site * 2u), eb = pload(pb, (site + TW) * 2u);
+        XY_CHECK(CHK_PARENT, ea < (uint32_t)(TW * TH * 2) && eb < (uint32_t)(TW * TH * 2) && !(ea & 1u) && !(eb & 1u));
+        sunion_v(pb, ea, eb);
     };
 #pragma unroll 1
     for (int j = 1; (1 << j) <= TH; ++j) {
@@ -793,6 +797,7 @@ k_label(const SweepArgs a)
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
             const uint32_t rl = root[v] >> 1;                            // byte offset -> tile-local index
+            XY_CHECK(CHK_PARENT, rl <= i0 + v);                         // a root is never after its site
             out[v] = gbase + (LabelT)(rl / TW) * (L - TW) + rl;          // row * L + col with row * TW + col = rl
             nib |= (rl == i0 + v) ? (1u << v) : 0u;
         }
@@ -943,7 +948,9 @@ k_flip(const SweepArgs a)
     while (merged) {
         const int b = __ffs(merged) - 1;
         merged &= merged - 1;
-        queue[atomicAdd(&nqueue, 1u)] = (uint16_t)(((b >> 2) * RPP + rq) * TW + 4 * q + (b & 3));
+        const uint32_t slot = atomicAdd(&nqueue, 1u);
+        XY_CHECK(CHK_QUEUE, slot < (uint32_t)(2 * (TW + TH)));
+        queue[slot] = (uint16_t)(((b >> 2) * RPP + rq) * TW + 4 * q + (b & 3));
     }
     __syncthreads();
     {
@@ -952,7 +959,7 @@ k_flip(const SweepArgs a)
             const uint32_t loc = queue[j];
             LabelT root = __ldg(labels + gbase + (LabelT)(loc / TW) * L + (loc % TW));
             LabelT p = __ldg(labels + root);
-            while (p != root) { root = p; p = __ldg(labels + root); }
+            while (p != root) { XY_CHECK(CHK_GLABEL, p < root); root = p; p = __ldg(labels + root); }
             const U4 c = rng(a.seed_lo, a.seed_hi, (uint64_t)root >> 7, a.t, TAG_FLIP);
             const uint32_t sel = ((uint32_t)root >> 5) & 3u;
             const uint32_t word = sel == 0 ? c.x : sel == 1 ? c.y : sel == 2 ? c.z : c.w;
@@ -981,6 +988,7 @@ k_flip(const SweepArgs a)
             const uint32_t d = (uint32_t)(lab[v] - gbase);              // r*L + c, < TH*L <= 2^22
             const uint32_t rr = __umulhi(d, a.Ldiv_mul) >> a.Ldiv_shift;
             const uint32_t loc = ((rb >> (4 * k + v)) & 1u) ? loc0 + v : d - rr * Lm;
+            XY_CHECK(CHK_LOC, loc < (uint32_t)(TW * TH));
             coins |= ((cbits[loc >> 5] >> (loc & 31u)) & 1u) << v;
         }
         if (coins) {                                                    // one branch per 4 sites; straight-line inside
