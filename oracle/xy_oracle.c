@@ -595,3 +595,118 @@ int xyo_run(float *theta, uint32_t L, uint64_t seed, uint64_t t0, double beta,
     free(bonds); free(label);
     return 0;
 }
+
+/* ========================================================================= */
+/* q-state Potts model on the same labeling / cluster-update core             */
+/* (PAPER.md:30-34 cites the authors' Potts / Ising SW     */
+/* codes, refs 19 and 22, without restating the rule: the textbook            */
+/* Swendsen-Wang update of PAPER.md:22's reference is used, readings P1-P5    */
+/* in DESIGN.md).                                                             */
+/*   H = -J sum_<ij> delta(s_i, s_j), J = 1, s_i in {0..q-1}, L x L periodic. */
+/*   P1 init   cold: all 0; hot: s_i = floor(q * w0 / 2^32), w = rng(seed, i, */
+/*             0, INIT).                                                      */
+/*   P2 bonds  bond <ij> active iff s_i == s_j and u < p, p = 1 - exp(-beta)  */
+/*             (fp64, -expm1(-beta)); u = the site's bond uniform of O1.      */
+/*   P3 label  O5 (minimum site index).                                       */
+/*   P4 spins  every cluster takes a fresh spin, uniform on {0..q-1}:         */
+/*             s = floor(q * w / 2^32), w = word (rho & 3) of                 */
+/*             rng(seed, rho >> 2, t, POTTS), rho the cluster's label.        */
+/*   P5 observe E = -#{links with equal spins} (x and y links), n_k = number  */
+/*             of sites with spin k.                                          */
+/* ========================================================================= */
+enum { XYO_TAG_POTTS = 5 };
+
+typedef struct {
+    uint64_t sweep;
+    double   beta;
+    int64_t  E;                 /* -(ex + ey) */
+    uint64_t ex, ey;            /* links with equal spins, per direction */
+    uint64_t count[16];         /* sites per spin value (q <= 16) */
+    uint64_t n_bonds_x, n_bonds_y, n_clusters;
+} xyo_potts_obs;
+
+int xyo_potts_init(uint8_t *spin, uint32_t L, uint32_t q, uint64_t seed, int init)
+{
+    uint64_t N = (uint64_t)L * L;
+    if (q < 2 || q > 16) return -1;
+    if (init == 0) { memset(spin, 0, N); return 0; }
+    if (init != 1) return -1;
+    for (uint64_t i = 0; i < N; ++i) {
+        uint32_t w[4];
+        xyo_rng(seed, i, 0, XYO_TAG_INIT, w);
+        spin[i] = (uint8_t)(((uint64_t)w[0] * q) >> 32);
+    }
+    return 0;
+}
+
+double xyo_potts_bond_prob(double beta) { return -expm1(-beta); }
+
+/* bonds[i]: bit0 = +x bond of site i, bit1 = +y bond */
+void xyo_potts_bonds(const uint8_t *spin, uint32_t L32, double beta, uint64_t seed, uint64_t t,
+                     uint8_t *bonds, uint64_t *nbx, uint64_t *nby)
+{
+    uint64_t L = L32, cx = 0, cy = 0;
+    double p = xyo_potts_bond_prob(beta);
+    for (uint64_t y = 0; y < L; ++y) {
+        for (uint64_t x = 0; x < L; ++x) {
+            uint64_t i = y * L + x;
+            double ux, uy;
+            uint8_t b = 0;
+            xyo_bond_uniforms_site(seed, t, i, &ux, &uy);
+            if (spin[i] == spin[right_of(x, y, L)] && ux < p) { b |= 1u; ++cx; }
+            if (spin[i] == spin[down_of(x, y, L)] && uy < p) { b |= 2u; ++cy; }
+            bonds[i] = b;
+        }
+    }
+    if (nbx) *nbx = cx;
+    if (nby) *nby = cy;
+}
+
+uint32_t xyo_potts_new_spin(uint64_t seed, uint64_t rho, uint64_t t, uint32_t q)
+{
+    uint32_t w[4];
+    xyo_rng(seed, rho >> 2, t, XYO_TAG_POTTS, w);
+    return (uint32_t)(((uint64_t)w[rho & 3u] * q) >> 32);
+}
+
+void xyo_potts_assign(uint8_t *spin, uint32_t L32, uint32_t q, const int64_t *label, uint64_t seed, uint64_t t)
+{
+    uint64_t N = (uint64_t)L32 * L32;
+    for (uint64_t i = 0; i < N; ++i)
+        spin[i] = (uint8_t)xyo_potts_new_spin(seed, (uint64_t)label[i], t, q);
+}
+
+void xyo_potts_observe(const uint8_t *spin, uint32_t L32, xyo_potts_obs *o)
+{
+    uint64_t L = L32;
+    o->ex = 0; o->ey = 0;
+    for (int k = 0; k < 16; ++k) o->count[k] = 0;
+    for (uint64_t y = 0; y < L; ++y) {
+        for (uint64_t x = 0; x < L; ++x) {
+            uint64_t i = y * L + x;
+            if (spin[i] == spin[right_of(x, y, L)]) ++o->ex;
+            if (spin[i] == spin[down_of(x, y, L)]) ++o->ey;
+            ++o->count[spin[i] & 15u];
+        }
+    }
+    o->E = -(int64_t)(o->ex + o->ey);
+}
+
+/* one sweep at counter t; bonds / label: caller-provided scratch of N entries; obs describes the */
+/* state AFTER the sweep, with the bond and cluster counts of this sweep                          */
+int xyo_potts_sweep(uint8_t *spin, uint32_t L, uint32_t q, uint64_t seed, uint64_t t, double beta,
+                    uint8_t *bonds, int64_t *label, xyo_potts_obs *obs)
+{
+    uint64_t nbx, nby, ncl;
+    if (q < 2 || q > 16) return -1;
+    xyo_potts_bonds(spin, L, beta, seed, t, bonds, &nbx, &nby);
+    ncl = xyo_label(bonds, L, label);
+    if (ncl == (uint64_t)-1) return -1;
+    xyo_potts_assign(spin, L, q, label, seed, t);
+    if (obs) {
+        xyo_potts_observe(spin, L, obs);
+        obs->sweep = t + 1; obs->beta = beta;
+        obs->n_bonds_x = nbx; obs->n_bonds_y = nby; obs->n_clusters = ncl;
+    }
+    return 0;
+}

@@ -291,3 +291,66 @@ def pcc_run(theta, L, seed, t0, beta0, sched: PccSchedule, trace_cap=0):
     return {"beta_final": out.beta_final, "dbeta_final": out.dbeta_final,
             "beta_mean": out.beta_mean, "n_decisions": int(out.n_decisions),
             "trace_len": int(out.trace_len), "trace_beta": tb[:n].copy(), "trace_bY": ty[:n].copy()}
+
+
+# ---------------------------------------------------------------------------------------------
+# q-state Potts model on the same labeling core (readings P1-P5 in xy_oracle.c)
+# ---------------------------------------------------------------------------------------------
+class PottsObs(C.Structure):
+    _fields_ = [("sweep", C.c_uint64), ("beta", C.c_double), ("E", C.c_int64),
+                ("ex", C.c_uint64), ("ey", C.c_uint64), ("count", C.c_uint64 * 16),
+                ("n_bonds_x", C.c_uint64), ("n_bonds_y", C.c_uint64), ("n_clusters", C.c_uint64)]
+
+
+TAG_POTTS = 5
+_potts_init = _sig("xyo_potts_init", C.c_int, [u8p, C.c_uint32, C.c_uint32, C.c_uint64, C.c_int])
+_potts_bond_prob = _sig("xyo_potts_bond_prob", C.c_double, [C.c_double])
+_potts_bonds = _sig("xyo_potts_bonds", None,
+                    [u8p, C.c_uint32, C.c_double, C.c_uint64, C.c_uint64, u8p, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)])
+_potts_new_spin = _sig("xyo_potts_new_spin", C.c_uint32, [C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint32])
+_potts_assign = _sig("xyo_potts_assign", None, [u8p, C.c_uint32, C.c_uint32, i64p, C.c_uint64, C.c_uint64])
+_potts_observe = _sig("xyo_potts_observe", None, [u8p, C.c_uint32, C.POINTER(PottsObs)])
+_potts_sweep = _sig("xyo_potts_sweep", C.c_int,
+                    [u8p, C.c_uint32, C.c_uint32, C.c_uint64, C.c_uint64, C.c_double, u8p, i64p, C.POINTER(PottsObs)])
+
+
+def potts_init(L, q, seed, kind):
+    spin = np.empty(L * L, np.uint8)
+    if _potts_init(spin, L, q, seed, kind) != 0:
+        raise ValueError("bad q or init kind")
+    return spin
+
+
+def potts_bond_prob(beta):
+    return _potts_bond_prob(beta)
+
+
+def potts_bonds(spin, L, beta, seed, t):
+    bonds = np.empty(L * L, np.uint8)
+    nx, ny = C.c_uint64(), C.c_uint64()
+    _potts_bonds(spin, L, beta, seed, t, bonds, C.byref(nx), C.byref(ny))
+    return bonds, nx.value, ny.value
+
+
+def potts_new_spin(seed, rho, t, q):
+    return _potts_new_spin(seed, int(rho), t, q)
+
+
+def potts_assign(spin, L, q, lab, seed, t):
+    _potts_assign(spin, L, q, np.ascontiguousarray(lab, np.int64), seed, t)
+
+
+def potts_observe(spin, L):
+    o = PottsObs()
+    _potts_observe(spin, L, C.byref(o))
+    return o
+
+
+def potts_sweep(spin, L, q, seed, t, beta):
+    """one sweep in place; returns (bonds, labels, obs)"""
+    bonds = np.empty(L * L, np.uint8)
+    lab = np.empty(L * L, np.int64)
+    o = PottsObs()
+    if _potts_sweep(spin, L, q, seed, t, beta, bonds, lab, C.byref(o)) != 0:
+        raise ValueError("potts sweep failed")
+    return bonds, lab, o
