@@ -202,6 +202,45 @@ int xy_debug_curand_philox(const uint32_t *ctr_host, const uint32_t *key_host, u
  * all zeros from the normal build, which compiles the checks away. */
 int xy_debug_check_counts(uint64_t counts[8], int *checked_build);
 
+/* ---- q-state Potts model on the same labeling core ------------------------
+ * PAPER.md:30-34 cites the authors' GPU Swendsen-Wang codes for the Potts and Ising models (refs 19, 22)
+ * as the origin of the labeling method; the update rule is not restated there and is the textbook one
+ * (readings P1-P5).  H = -J sum_<ij> delta(s_i, s_j), J = 1, s_i in {0..q-1} held as
+ * one byte per site, L x L periodic, same site and bond indexing as above.  One sweep at counter t:
+ *   bonds  <ij> active iff s_i == s_j and u < 1 - exp(-beta), u the site's bond uniform of the XY sweep;
+ *   labels as above (k_label / k_merge unchanged);
+ *   spins  every cluster takes s = floor(q w / 2^32), w = word (rho & 3) of Philox(seed; rho >> 2, t, POTTS),
+ *          rho the cluster's label.
+ * q = 2 is the Ising model at coupling beta / 2.  Labels are 32-bit.  Same error codes as above. */
+typedef struct xy_potts xy_potts;   /* opaque */
+
+typedef struct {
+    uint64_t sweep;                 /* T: sweeps done */
+    double   beta;                  /* beta of sweep T-1 (NaN before the first sweep) */
+    int64_t  E;                     /* -(ex + ey) */
+    uint64_t ex, ey;                /* x / y links with equal spins in the current configuration */
+    uint64_t count[16];             /* sites per spin value (entries >= q are 0) */
+    uint64_t n_bonds_x, n_bonds_y, n_clusters;   /* of sweep T-1 (0 before the first sweep) */
+} xy_potts_obs;
+
+/* L as for xy_create; 2 <= q <= 16; init XY_INIT_COLD (all 0) or XY_INIT_HOT (s_i = floor(q w0 / 2^32) of the
+ * INIT call of site i).  The library allocates the device workspace (about 5.4 bytes per site + 16 MiB). */
+int xy_potts_create(xy_potts **out, uint32_t L, uint32_t q, uint64_t seed, int init);
+int xy_potts_destroy(xy_potts *s);
+/* n sweeps at beta (finite, >= 0), enqueued on cuda_stream (cudaStream_t, NULL = default); does not block. */
+int xy_potts_sweeps(xy_potts *s, double beta, uint64_t n, void *cuda_stream);
+/* observables of the current configuration (one counting pass); blocks until the stream is idle */
+int xy_potts_measure(xy_potts *s, xy_potts_obs *out);
+/* host buffers: the first n spins (n <= L*L); all L*L spins, rejected with XY_ERR_ARG (state unchanged) if any is >= q */
+int xy_potts_get_spins(xy_potts *s, uint8_t *host, size_t n);
+int xy_potts_set_spins(xy_potts *s, const uint8_t *host, size_t n);
+int xy_potts_get_sweep(xy_potts *s, uint64_t *t);
+int xy_potts_set_sweep(xy_potts *s, uint64_t t);
+/* bonds (byte per site: bit0 = +x, bit1 = +y) and canonical labels (minimum site index) of the last sweep */
+int xy_potts_get_bonds(xy_potts *s, uint8_t *host, size_t n);
+int xy_potts_get_labels(xy_potts *s, int64_t *host, size_t n);
+int xy_potts_get_launch_count(xy_potts *s, uint64_t *count);
+
 const char *xy_last_error(void);
 
 #ifdef __cplusplus

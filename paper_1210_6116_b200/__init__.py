@@ -8,7 +8,8 @@ The binding is loaded on first use so that `paper_1210_6116_b200.build` (which p
 library) can be imported before the library exists.
 """
 __all__ = ["XYState", "XYError", "Obs", "PccSchedule", "OBS_DTYPE", "INIT_COLD", "INIT_HOT", "OBS_NONE", "OBS_ALL",
-           "FLAG_LABELS64", "FLAG_FOURIER", "Fourier", "FOURIER_DTYPE", "workspace_bytes", "debug_philox", "debug_check_counts", "debug_curand_philox", "lib_path"]
+           "FLAG_LABELS64", "FLAG_FOURIER", "Fourier", "FOURIER_DTYPE", "workspace_bytes", "debug_philox", "debug_check_counts", "debug_curand_philox", "lib_path",
+           "PottsState", "PottsObs"]
 
 
 def __getattr__(name):

@@ -107,6 +107,17 @@ _SIGS = {
     "xy_get_launch_count": [_vp, C.POINTER(C.c_uint64)],
     "xy_label_bonds": [_vp, _vp, C.c_size_t],
     "xy_debug_check_counts": [C.POINTER(C.c_uint64), C.POINTER(C.c_int)],
+    "xy_potts_create": [C.POINTER(_vp), C.c_uint32, C.c_uint32, C.c_uint64, C.c_int],
+    "xy_potts_destroy": [_vp],
+    "xy_potts_sweeps": [_vp, C.c_double, C.c_uint64, _vp],
+    "xy_potts_measure": [_vp, _vp],
+    "xy_potts_get_spins": [_vp, _vp, C.c_size_t],
+    "xy_potts_set_spins": [_vp, _vp, C.c_size_t],
+    "xy_potts_get_sweep": [_vp, C.POINTER(C.c_uint64)],
+    "xy_potts_set_sweep": [_vp, C.c_uint64],
+    "xy_potts_get_bonds": [_vp, _vp, C.c_size_t],
+    "xy_potts_get_labels": [_vp, _vp, C.c_size_t],
+    "xy_potts_get_launch_count": [_vp, C.POINTER(C.c_uint64)],
     "xy_debug_philox": [_vp, _vp, _vp, C.c_size_t],
     "xy_debug_curand_philox": [_vp, _vp, _vp, C.c_size_t],
 }
@@ -308,3 +319,74 @@ def debug_philox(ctr, key):
 
 def debug_curand_philox(ctr, key):
     return _philox_common(_lib.xy_debug_curand_philox, ctr, key)
+
+
+# ---------------------------------------------------------------------------------------------
+# q-state Potts model on the same labeling core (include/xy.h, section "Potts")
+# ---------------------------------------------------------------------------------------------
+class PottsObs(C.Structure):
+    _fields_ = [("sweep", C.c_uint64), ("beta", C.c_double), ("E", C.c_int64),
+                ("ex", C.c_uint64), ("ey", C.c_uint64), ("count", C.c_uint64 * 16),
+                ("n_bonds_x", C.c_uint64), ("n_bonds_y", C.c_uint64), ("n_clusters", C.c_uint64)]
+
+
+class PottsState:
+    """Owner of one xy_potts (marshalling only)."""
+
+    def __init__(self, L, q, seed, init=INIT_HOT):
+        self._h = _vp()
+        self.L, self.q, self.N = L, q, L * L
+        _check(_lib.xy_potts_create(C.byref(self._h), L, q, seed, init))
+
+    def destroy(self):
+        if self._h:
+            _check(_lib.xy_potts_destroy(self._h))
+            self._h = _vp()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def sweeps(self, beta, n=1, stream=None):
+        import torch
+        st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+        _check(_lib.xy_potts_sweeps(self._h, beta, n, st))
+
+    def measure(self):
+        o = PottsObs()
+        _check(_lib.xy_potts_measure(self._h, C.byref(o)))
+        return o
+
+    def get_spins(self, n=None):
+        out = np.empty(self.N if n is None else n, np.uint8)
+        _check(_lib.xy_potts_get_spins(self._h, out.ctypes.data, out.size))
+        return out
+
+    def set_spins(self, spins):
+        a = np.ascontiguousarray(spins, np.uint8)
+        _check(_lib.xy_potts_set_spins(self._h, a.ctypes.data, a.size))
+
+    def get_sweep(self):
+        t = C.c_uint64()
+        _check(_lib.xy_potts_get_sweep(self._h, C.byref(t)))
+        return t.value
+
+    def set_sweep(self, t):
+        _check(_lib.xy_potts_set_sweep(self._h, t))
+
+    def get_bonds(self, n=None):
+        out = np.empty(self.N if n is None else n, np.uint8)
+        _check(_lib.xy_potts_get_bonds(self._h, out.ctypes.data, out.size))
+        return out
+
+    def get_labels(self, n=None):
+        out = np.empty(self.N if n is None else n, np.int64)
+        _check(_lib.xy_potts_get_labels(self._h, out.ctypes.data, out.size))
+        return out
+
+    def get_launch_count(self):
+        c = C.c_uint64()
+        _check(_lib.xy_potts_get_launch_count(self._h, C.byref(c)))
+        return c.value

@@ -1,0 +1,227 @@
+// potts_kernels.cuh -- q-state Potts Swendsen-Wang sweep on the labeling core of the XY sweep (
+// PAPER.md:30-34 names the authors' Potts / Ising SW codes).  H = -sum_<ij> delta(s_i, s_j), spins one byte per site.
+//   k_potts_bonds  (P2, and P5 of the incoming configuration): bond <ij> active iff s_i == s_j and u < 1 - exp(-beta);
+//                  the same Philox bond uniforms and the same nibble-packed bond bytes as k_bonds, so that
+//                  k_label / k_merge run unchanged.  u < p is an integer compare: u = (w + 0.5) 2^-32 < p
+//                  <=> w < T, T = ceil(p 2^32 - 0.5) (host, exact in fp64).  The 16 leading bits of w (call A of
+//                  the quad) settle it unless they equal T >> 16; only then call B is drawn.
+//   k_potts_flip   (P4): every tile-local root takes the fresh spin of its cluster's canonical label (one Philox
+//                  call serves 4 consecutive labels), chasing to the global root if k_merge linked it elsewhere;
+//                  every other site copies the spin of its tile root from shared memory.
+// Product code: shares nothing with oracle/.
+#pragma once
+#include "xy_kernels.cuh"
+
+namespace xy {
+
+constexpr uint32_t TAG_POTTS = 5;
+constexpr int kPottsMaxQ = 16;
+
+// integer observables and counters of the Potts state (all sums are exact, so plain atomics are reproducible)
+struct PottsCtl {
+    unsigned long long ex, ey;                 // links with equal spins (incoming state of the last k_potts_bonds)
+    unsigned long long count[kPottsMaxQ];      // sites per spin value
+    unsigned long long nbx, nby, ncl;          // bonds and clusters of the last sweep
+};
+
+struct PottsArgs {
+    uint8_t  *spin;
+    uint8_t  *bonds;
+    PottsCtl *ctl;
+    uint32_t  L, q;
+    uint32_t  seed_lo, seed_hi, t;
+    uint64_t  T;                               // threshold: bond iff equal spins and w < T (0 .. 2^32)
+};
+
+__device__ __forceinline__ uint32_t eq4_bits(uint32_t a, uint32_t b)   // bit j = byte j of a equals byte j of b
+{
+    const uint32_t m = __vcmpeq4(a, b) & 0x01010101u;
+    return (m | (m >> 7) | (m >> 14) | (m >> 21)) & 15u;
+}
+
+// kBonds = false: observables only (xy_potts_measure of a state no sweep has looked at yet)
+template <bool kBonds>
+__global__ void __launch_bounds__(256)
+k_potts_bonds(const PottsArgs a)
+{
+    const uint32_t L = a.L, q = a.q;
+    const uint64_t nquads = ((uint64_t)L * L) >> 2;
+    const uint32_t Th = (uint32_t)(a.T >> 16), Tl = (uint32_t)(a.T & 0xffffu);
+    unsigned long long ex = 0, ey = 0, nbx = 0, nby = 0;
+    uint32_t cnt[kPottsMaxQ];
+#pragma unroll
+    for (int k = 0; k < kPottsMaxQ; ++k) cnt[k] = 0;
+
+    for (uint64_t qd = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; qd < nquads; qd += (uint64_t)gridDim.x * blockDim.x) {
+        const uint64_t i0 = qd << 2;
+        const uint32_t y = (uint32_t)(i0 / L), x = (uint32_t)(i0 - (uint64_t)y * L);
+        const uint32_t own = __ldg(reinterpret_cast<const uint32_t *>(a.spin + i0));
+        const uint32_t xr = x + 4 == L ? 0u : x + 4;
+        const uint32_t nb = __ldg(a.spin + (uint64_t)y * L + xr);
+        const uint32_t yd = y + 1 == L ? 0u : y + 1;
+        const uint32_t down = __ldg(reinterpret_cast<const uint32_t *>(a.spin + (uint64_t)yd * L + x));
+        const uint32_t eqx = eq4_bits(own, (own >> 8) | (nb << 24));
+        const uint32_t eqy = eq4_bits(own, down);
+        ex += __popc(eqx);
+        ey += __popc(eqy);
+#pragma unroll
+        for (int k = 0; k < kPottsMaxQ; ++k)
+            if (k < (int)q) cnt[k] += __popc(__vcmpeq4(own, 0x01010101u * (uint32_t)k) & 0x01010101u);
+        if constexpr (kBonds) {
+            const U4 wA = rng(a.seed_lo, a.seed_hi, qd, a.t, TAG_BOND);
+            const uint32_t w[4] = {wA.x, wA.y, wA.z, wA.w};
+            uint32_t xn = 0, yn = 0, open = 0;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const uint32_t hx = w[j] & 0xffffu, hy = w[j] >> 16;
+                xn |= (hx < Th ? 1u : 0u) << j;
+                yn |= (hy < Th ? 1u : 0u) << j;
+                open |= (hx == Th ? 1u : 0u) << j;
+                open |= (hy == Th ? 16u : 0u) << j;
+            }
+            if (open & (eqx | (eqy << 4))) {               // rare (2^-16 per decision): the trailing 16 bits decide
+                const U4 wB = rng(a.seed_lo, a.seed_hi, qd, a.t, TAG_BOND_LO);
+                const uint32_t v[4] = {wB.x, wB.y, wB.z, wB.w};
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    if ((open >> j) & 1u) xn |= ((v[j] & 0xffffu) < Tl ? 1u : 0u) << j;
+                    if ((open >> (4 + j)) & 1u) yn |= ((v[j] >> 16) < Tl ? 1u : 0u) << j;
+                }
+            }
+            xn &= eqx;
+            yn &= eqy;
+            nbx += __popc(xn);
+            nby += __popc(yn);
+            a.bonds[qd] = (uint8_t)(xn | (yn << 4));
+        }
+    }
+    ex = warp_sum_u64(ex); ey = warp_sum_u64(ey);
+    nbx = warp_sum_u64(nbx); nby = warp_sum_u64(nby);
+    unsigned long long c64[kPottsMaxQ];
+#pragma unroll
+    for (int k = 0; k < kPottsMaxQ; ++k) c64[k] = k < (int)q ? warp_sum_u64(cnt[k]) : 0ull;
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(&a.ctl->ex, ex);
+        atomicAdd(&a.ctl->ey, ey);
+#pragma unroll
+        for (int k = 0; k < kPottsMaxQ; ++k)
+            if (k < (int)q && c64[k]) atomicAdd(&a.ctl->count[k], c64[k]);
+        if constexpr (kBonds) {
+            atomicAdd(&a.ctl->nbx, nbx);
+            atomicAdd(&a.ctl->nby, nby);
+        }
+    }
+}
+
+__device__ __forceinline__ uint32_t potts_draw(uint32_t seed_lo, uint32_t seed_hi, uint64_t rho, uint32_t t, uint32_t q)
+{
+    const U4 c = rng(seed_lo, seed_hi, rho >> 2, t, TAG_POTTS);
+    const uint32_t sel = (uint32_t)rho & 3u;
+    const uint32_t w = sel == 0 ? c.x : sel == 1 ? c.y : sel == 2 ? c.z : c.w;
+    return __umulhi(w, q);                                              // floor(q w / 2^32)
+}
+
+// One CTA per TW x TH tile (the tiles of k_label), 4 consecutive sites x TH/RPP rows per thread.
+template <int WPR, int TH, typename LabelT>
+__global__ void __launch_bounds__(WPR * TH)
+k_potts_flip(const SweepArgs a, const PottsArgs p)
+{
+    constexpr int TW = 32 * WPR, NT = WPR * TH;
+    constexpr int Q = TW / 4, RPP = NT / Q, NP = TH / RPP;
+    __shared__ uint8_t fresh[TW * TH];               // fresh spin of the tile root at tile-local index loc
+    __shared__ unsigned long long sc[NT / 32];
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t L = a.L;
+    const LabelT *labels = reinterpret_cast<const LabelT *>(a.labels);
+    const uint32_t tile = blockIdx.x;
+    const uint32_t ty = tile / a.tiles_x, tx = tile - ty * a.tiles_x;
+    const uint32_t x0 = tx * TW, y0 = ty * TH;
+    const int q4 = tid % Q, rq = tid / Q;
+    const LabelT gbase = (LabelT)y0 * L + x0;
+
+    auto load_labels = [&](size_t i, LabelT (&lab)[4]) {
+        if constexpr (sizeof(LabelT) == 4) {
+            const uint4 v = __ldg(reinterpret_cast<const uint4 *>(labels + i));
+            lab[0] = v.x; lab[1] = v.y; lab[2] = v.z; lab[3] = v.w;
+        } else {
+            const ulonglong2 u = __ldg(reinterpret_cast<const ulonglong2 *>(labels + i));
+            const ulonglong2 v = __ldg(reinterpret_cast<const ulonglong2 *>(labels + i + 2));
+            lab[0] = u.x; lab[1] = u.y; lab[2] = v.x; lab[3] = v.y;
+        }
+    };
+
+    // ---- tile roots draw (their own label if it still is a global root, else the root k_merge linked them to) ----
+    uint32_t rb = 0, ncl = 0;
+#pragma unroll 1
+    for (int k = 0; k < NP; ++k) {
+        const int row = k * RPP + rq;
+        const size_t i = (size_t)(y0 + row) * L + x0 + 4 * q4;
+        LabelT lab[4];
+        load_labels(i, lab);
+        const uint32_t nib = (__ldg(reinterpret_cast<const uint8_t *>(a.rootmask) + (i >> 3)) >> (i & 4u)) & 15u;
+        rb |= nib << (4 * k);
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+            if ((nib >> v) & 1u) {
+                LabelT root = lab[v];
+                if (root == (LabelT)(i + v)) {
+                    ++ncl;
+                } else {                                                 // read-only chase: the forest is final
+                    LabelT up = __ldg(labels + root);
+                    while (up != root) { XY_CHECK(CHK_GLABEL, up < root); root = up; up = __ldg(labels + root); }
+                }
+                fresh[row * TW + 4 * q4 + v] = (uint8_t)potts_draw(p.seed_lo, p.seed_hi, (uint64_t)root, p.t, p.q);
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---- every site takes the fresh spin of its tile root ----
+    const uint32_t Lm = L - TW;
+#pragma unroll
+    for (int k = 0; k < NP; ++k) {
+        const int row = k * RPP + rq;
+        const uint32_t loc0 = row * TW + 4 * q4;
+        const size_t i = (size_t)(y0 + row) * L + x0 + 4 * q4;
+        LabelT lab[4];
+        load_labels(i, lab);
+        uint32_t out = 0;
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+            const uint32_t d = (uint32_t)(lab[v] - gbase);              // r*L + c, < TH*L <= 2^22
+            const uint32_t rr = __umulhi(d, a.Ldiv_mul) >> a.Ldiv_shift;
+            const uint32_t loc = ((rb >> (4 * k + v)) & 1u) ? loc0 + v : d - rr * Lm;
+            XY_CHECK(CHK_LOC, loc < (uint32_t)(TW * TH));
+            out |= (uint32_t)fresh[loc] << (8 * v);
+        }
+        *reinterpret_cast<uint32_t *>(p.spin + i) = out;
+    }
+
+    unsigned long long c = warp_sum_u64(ncl);
+    if (lane == 0) sc[warp] = c;
+    __syncthreads();
+    if (tid == 0) {
+        unsigned long long tot = 0;
+        for (int w = 0; w < NT / 32; ++w) tot += sc[w];
+        atomicAdd(&p.ctl->ncl, tot);
+    }
+}
+
+__global__ void k_potts_init_hot(uint8_t *spin, uint64_t N, uint32_t q, uint32_t seed_lo, uint32_t seed_hi)
+{
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (uint64_t)gridDim.x * blockDim.x) {
+        const U4 w = rng(seed_lo, seed_hi, i, 0u, TAG_INIT);
+        spin[i] = (uint8_t)__umulhi(w.x, q);
+    }
+}
+
+__global__ void k_potts_check_spins(const uint8_t *spin, uint64_t N, uint32_t q, unsigned int *flag)
+{
+    bool bad = false;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (uint64_t)gridDim.x * blockDim.x)
+        bad |= spin[i] >= q;
+    if (bad) atomicOr(flag, 1u);
+}
+
+}  // namespace xy

@@ -288,6 +288,17 @@ int check_L(uint32_t L)
     return XY_OK;
 }
 
+// d / L for d < 2^22 (k_flip): with 2^sh <= L < 2^(sh+1), M = ceil(2^(31+sh) / L) <= 2^31 and
+// floor(d M / 2^(31+sh)) = floor(d / L) because the excess d e / 2^(31+sh) < 2^(-9-sh) < 1/L
+void set_Ldiv(SweepArgs &a, uint32_t L)
+{
+    uint32_t sh = 0;
+    while ((2u << sh) <= L) ++sh;
+    const uint64_t num = 1ull << (31 + sh);
+    a.Ldiv_mul = (uint32_t)((num + L - 1) / L);
+    a.Ldiv_shift = sh - 1;
+}
+
 SweepArgs base_args(const xy_state *s)
 {
     SweepArgs a;
@@ -303,15 +314,7 @@ SweepArgs base_args(const xy_state *s)
     a.L = s->L;
     a.tiles_x = s->L / s->ker.tw;
     a.ntiles = a.tiles_x * (s->L / s->ker.th);
-    {
-        // d / L for d < 2^22 (k_flip): with 2^sh <= L < 2^(sh+1), M = ceil(2^(31+sh) / L) <= 2^31 and
-        // floor(d M / 2^(31+sh)) = floor(d / L) because the excess d e / 2^(31+sh) < 2^(-9-sh) < 1/L
-        uint32_t sh = 0;
-        while ((2u << sh) <= s->L) ++sh;
-        const uint64_t num = 1ull << (31 + sh);
-        a.Ldiv_mul = (uint32_t)((num + s->L - 1) / s->L);
-        a.Ldiv_shift = sh - 1;
-    }
+    set_Ldiv(a, s->L);
     a.seed_lo = (uint32_t)(s->seed & 0xffffffffu);
     a.seed_hi = (uint32_t)(s->seed >> 32);
     for (uint32_t r = 0; r < 10; ++r) {
@@ -990,3 +993,5 @@ int xy_debug_curand_philox(const uint32_t *ctr, const uint32_t *key, uint32_t *o
 }
 
 }  // extern "C"
+
+#include "potts_api.cuh"
