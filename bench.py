@@ -257,6 +257,34 @@ def labeling_only(xy, torch, L, kinds=("all_on", "h_stripes", "serpentine"), rep
     return out
 
 
+def potts_leg(xy, torch, L=16384, q=3, seed=13, therm=100, K=50):
+    """q-state Potts sweep at the self-dual point beta_c = ln(1 + sqrt q): the XY sweep's
+    k_label / k_merge between k_potts_bonds and k_potts_flip; u32 labels, one byte per spin."""
+    import math
+    beta = math.log(1.0 + math.sqrt(q))
+    N = L * L
+    st = xy.PottsState(L, q, seed, xy.INIT_HOT)
+    st.sweeps(beta, therm)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    st.sweeps(beta, K)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    o = st.measure()
+    st.destroy()
+    torch.cuda.empty_cache()
+    # spins 1 B read (+ halo re-reads from L2) and bits 0.25 written; label pass as in the XY sweep; flip: labels 4,
+    # root bits 0.125, spins 1 written
+    bps = (1.0 + 0.25) + (0.25 + 4 + 0.125) + (128 + 32) * (2 * 4 + 0.125) / (128 * 32) + (4 + 0.125 + 1.0)
+    peak, _ = measured_peaks()
+    return {"L": L, "q": q, "beta": beta, "untimed_sweeps": therm, "steps": K, "ms_per_step": ms / K,
+            "updates_per_s": N * K / (ms * 1e-3), "bytes_per_site": bps,
+            "sweep_roofline_frac": bps * N * K / (ms * 1e-3) / 1e9 / peak,
+            "E_per_site": o.E / N, "bond_density": (o.n_bonds_x + o.n_bonds_y) / (2 * N), "clusters_per_site": o.n_clusters / N}
+
+
 def run_reference(args, rank, world):
     """--impl reference: the CPU oracle timed on the host cores (rank 0 only)."""
     if rank != 0:
@@ -497,6 +525,7 @@ def main():
             "cfg5_L65536_i64_observables_off": timed_leg(xy, torch, c5[1], c5[2], c5[3], c5[4], flags=xy.FLAG_LABELS64,
                                                          warm=20, K=20, obs="none"),
             "labeling_only_L16384": labeling_only(xy, torch, 16384),
+            "potts_q3_L16384": potts_leg(xy, torch),
             "note": "value / ms_per_step above are config 4 with all six sums on; entries here are labelled variants, "
                     "never the headline.  cfg5 is timed from the hot start as BASELINE config 5 states (its first "
                     "sweeps are transient: see per_sweep_ms)",

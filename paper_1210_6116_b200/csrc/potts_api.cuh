@@ -69,11 +69,13 @@ void potts_flip_launch(const xy_potts *s, const SweepArgs &a, const PottsArgs &p
     else k_potts_flip<2, kR * kNW, uint32_t><<<a.ntiles, 2 * kR * kNW, 0, s->stream>>>(a, p);
 }
 
-int potts_grid(uint64_t work_items)
+template <bool kB>
+void potts_bonds_launch(const xy_potts *s, const PottsArgs &p)
 {
-    uint64_t b = (work_items + 255) / 256;
-    if (b > 148ull * 16) b = 148ull * 16;
-    return (int)(b ? b : 1);
+    const int grid = 148 * 8;
+    if (s->q <= 4) k_potts_bonds<kB, 4><<<grid, 256, 0, s->stream>>>(p);
+    else if (s->q <= 8) k_potts_bonds<kB, 8><<<grid, 256, 0, s->stream>>>(p);
+    else k_potts_bonds<kB, 16><<<grid, 256, 0, s->stream>>>(p);
 }
 
 }  // namespace
@@ -157,7 +159,7 @@ int xy_potts_sweeps(xy_potts *s, double beta, uint64_t n, void *cuda_stream)
     for (uint64_t k = 0; k < n; ++k) {
         const PottsArgs p = potts_args(s, beta);
         CUDA_TRY(cudaMemsetAsync(s->ctl(), 0, sizeof(PottsCtl), s->stream));
-        k_potts_bonds<true><<<potts_grid(s->N / 4), 256, 0, s->stream>>>(p);
+        potts_bonds_launch<true>(s, p);
         s->ker.label(a, s->stream);
         s->ker.merge(a, s->stream);
         potts_flip_launch(s, a, p);
@@ -179,7 +181,7 @@ int xy_potts_measure(xy_potts *s, xy_potts_obs *out)
     CUDA_TRY(cudaStreamSynchronize(s->stream));
     const unsigned long long nbx = h.nbx, nby = h.nby, ncl = h.ncl;
     CUDA_TRY(cudaMemsetAsync(s->ctl(), 0, sizeof(PottsCtl), s->stream));
-    k_potts_bonds<false><<<potts_grid(s->N / 4), 256, 0, s->stream>>>(potts_args(s, 0.0));
+    potts_bonds_launch<false>(s, potts_args(s, 0.0));
     CUDA_TRY(cudaGetLastError());
     s->launches += 1;
     CUDA_TRY(cudaMemcpyAsync(&h, s->ctl(), sizeof h, cudaMemcpyDeviceToHost, s->stream));

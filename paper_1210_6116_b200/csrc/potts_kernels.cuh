@@ -39,22 +39,23 @@ __device__ __forceinline__ uint32_t eq4_bits(uint32_t a, uint32_t b)   // bit j 
     return (m | (m >> 7) | (m >> 14) | (m >> 21)) & 15u;
 }
 
-// kBonds = false: observables only (xy_potts_measure of a state no sweep has looked at yet)
-template <bool kBonds>
+// kBonds = false: observables only (xy_potts_measure of a state no sweep has looked at yet).  KQ: number of spin
+// values counted (q <= KQ; 4, 8 or 16).  A thread owns quads of 4 consecutive sites (one bond byte, one Philox call).
+template <bool kBonds, int KQ>
 __global__ void __launch_bounds__(256)
 k_potts_bonds(const PottsArgs a)
 {
     const uint32_t L = a.L, q = a.q;
-    const uint64_t nquads = ((uint64_t)L * L) >> 2;
+    const uint32_t nquads = (uint32_t)(((uint64_t)L * L) >> 2), qpr = L >> 2;      // quads in all, per row
     const uint32_t Th = (uint32_t)(a.T >> 16), Tl = (uint32_t)(a.T & 0xffffu);
     unsigned long long ex = 0, ey = 0, nbx = 0, nby = 0;
-    uint32_t cnt[kPottsMaxQ];
+    uint32_t cnt[KQ];
 #pragma unroll
-    for (int k = 0; k < kPottsMaxQ; ++k) cnt[k] = 0;
+    for (int k = 0; k < KQ; ++k) cnt[k] = 0;
 
-    for (uint64_t qd = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; qd < nquads; qd += (uint64_t)gridDim.x * blockDim.x) {
-        const uint64_t i0 = qd << 2;
-        const uint32_t y = (uint32_t)(i0 / L), x = (uint32_t)(i0 - (uint64_t)y * L);
+    for (uint32_t qd = blockIdx.x * blockDim.x + threadIdx.x; qd < nquads; qd += gridDim.x * blockDim.x) {
+        const uint64_t i0 = (uint64_t)qd << 2;
+        const uint32_t y = qd / qpr, x = (qd - y * qpr) << 2;
         const uint32_t own = __ldg(reinterpret_cast<const uint32_t *>(a.spin + i0));
         const uint32_t xr = x + 4 == L ? 0u : x + 4;
         const uint32_t nb = __ldg(a.spin + (uint64_t)y * L + xr);
@@ -65,8 +66,7 @@ k_potts_bonds(const PottsArgs a)
         ex += __popc(eqx);
         ey += __popc(eqy);
 #pragma unroll
-        for (int k = 0; k < kPottsMaxQ; ++k)
-            if (k < (int)q) cnt[k] += __popc(__vcmpeq4(own, 0x01010101u * (uint32_t)k) & 0x01010101u);
+        for (int k = 0; k < KQ; ++k) cnt[k] += __popc(__vcmpeq4(own, 0x01010101u * (uint32_t)k) & 0x01010101u);
         if constexpr (kBonds) {
             const U4 wA = rng(a.seed_lo, a.seed_hi, qd, a.t, TAG_BOND);
             const uint32_t w[4] = {wA.x, wA.y, wA.z, wA.w};
@@ -97,14 +97,14 @@ k_potts_bonds(const PottsArgs a)
     }
     ex = warp_sum_u64(ex); ey = warp_sum_u64(ey);
     nbx = warp_sum_u64(nbx); nby = warp_sum_u64(nby);
-    unsigned long long c64[kPottsMaxQ];
+    unsigned long long c64[KQ];
 #pragma unroll
-    for (int k = 0; k < kPottsMaxQ; ++k) c64[k] = k < (int)q ? warp_sum_u64(cnt[k]) : 0ull;
+    for (int k = 0; k < KQ; ++k) c64[k] = warp_sum_u64(cnt[k]);
     if ((threadIdx.x & 31) == 0) {
         atomicAdd(&a.ctl->ex, ex);
         atomicAdd(&a.ctl->ey, ey);
 #pragma unroll
-        for (int k = 0; k < kPottsMaxQ; ++k)
+        for (int k = 0; k < KQ; ++k)
             if (k < (int)q && c64[k]) atomicAdd(&a.ctl->count[k], c64[k]);
         if constexpr (kBonds) {
             atomicAdd(&a.ctl->nbx, nbx);
@@ -129,6 +129,8 @@ k_potts_flip(const SweepArgs a, const PottsArgs p)
     constexpr int TW = 32 * WPR, NT = WPR * TH;
     constexpr int Q = TW / 4, RPP = NT / Q, NP = TH / RPP;
     __shared__ uint8_t fresh[TW * TH];               // fresh spin of the tile root at tile-local index loc
+    __shared__ uint16_t queue[TW * TH];              // tile-local indices of the tile roots
+    __shared__ uint32_t nqueue;
     __shared__ unsigned long long sc[NT / 32];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -151,29 +153,47 @@ k_potts_flip(const SweepArgs a, const PottsArgs p)
         }
     };
 
-    // ---- tile roots draw (their own label if it still is a global root, else the root k_merge linked them to) ----
+    // ---- tile roots are queued (a tile has TW*TH of them at most), then draw densely: their own label if it still
+    //      is a global root, else the root k_merge linked them to ----
+    if (tid == 0) nqueue = 0;
+    __syncthreads();
     uint32_t rb = 0, ncl = 0;
-#pragma unroll 1
-    for (int k = 0; k < NP; ++k) {
-        const int row = k * RPP + rq;
-        const size_t i = (size_t)(y0 + row) * L + x0 + 4 * q4;
-        LabelT lab[4];
-        load_labels(i, lab);
-        const uint32_t nib = (__ldg(reinterpret_cast<const uint8_t *>(a.rootmask) + (i >> 3)) >> (i & 4u)) & 15u;
-        rb |= nib << (4 * k);
 #pragma unroll
-        for (int v = 0; v < 4; ++v) {
-            if ((nib >> v) & 1u) {
-                LabelT root = lab[v];
-                if (root == (LabelT)(i + v)) {
-                    ++ncl;
-                } else {                                                 // read-only chase: the forest is final
-                    LabelT up = __ldg(labels + root);
-                    while (up != root) { XY_CHECK(CHK_GLABEL, up < root); root = up; up = __ldg(labels + root); }
-                }
-                fresh[row * TW + 4 * q4 + v] = (uint8_t)potts_draw(p.seed_lo, p.seed_hi, (uint64_t)root, p.t, p.q);
-            }
+    for (int k = 0; k < NP; ++k) {
+        const size_t i = (size_t)(y0 + k * RPP + rq) * L + x0 + 4 * q4;
+        rb |= ((__ldg(reinterpret_cast<const uint8_t *>(a.rootmask) + (i >> 3)) >> (i & 4u)) & 15u) << (4 * k);
+    }
+    {
+        // one slot reservation per warp: ballots of the four-bit counts
+        const uint32_t n = __popc(rb);
+        uint32_t pre = n;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, pre, o);
+            if (lane >= o) pre += t;
         }
+        uint32_t wbase = 0;
+        if (lane == 31) wbase = atomicAdd(&nqueue, pre);
+        wbase = __shfl_sync(0xffffffffu, wbase, 31);
+        uint32_t slot = wbase + pre - n, bits = rb;
+        while (bits) {
+            const int b = __ffs(bits) - 1;
+            bits &= bits - 1;
+            queue[slot++] = (uint16_t)(((b >> 2) * RPP + rq) * TW + 4 * q4 + (b & 3));
+        }
+    }
+    __syncthreads();
+    for (uint32_t j = tid; j < nqueue; j += NT) {
+        const uint32_t loc = queue[j];
+        const LabelT self = gbase + (LabelT)(loc / TW) * L + (loc % TW);
+        LabelT root = __ldg(labels + self);
+        if (root == self) {
+            ++ncl;
+        } else {                                                         // read-only chase: the forest is final
+            LabelT up = __ldg(labels + root);
+            while (up != root) { XY_CHECK(CHK_GLABEL, up < root); root = up; up = __ldg(labels + root); }
+        }
+        fresh[loc] = (uint8_t)potts_draw(p.seed_lo, p.seed_hi, (uint64_t)root, p.t, p.q);
     }
     __syncthreads();
 
