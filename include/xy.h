@@ -202,6 +202,31 @@ int xy_debug_curand_philox(const uint32_t *ctr_host, const uint32_t *key_host, u
  * all zeros from the normal build, which compiles the checks away. */
 int xy_debug_check_counts(uint64_t counts[8], int *checked_build);
 
+/* ---- row-slab sharding across GPUs (SURVEY.md 8(e) / 8(f) #3; PAPER.md:34 "the inter-GPU labeling", :64) ----------
+ * One state per rank holds rows [y_off, y_off + rows) of the L x L lattice (rows and y_off multiples of 32, fewer than
+ * 2^31 sites, 32-bit labels) plus one halo row: the first row of the slab below (of rank 0 for the last rank).  Every
+ * random number is keyed by the site's index in the WHOLE lattice, so G slabs reproduce the sweep of one L x L state
+ * bit for bit.  One sweep at counter t is
+ *     xy_slab_label   (every rank)  direction, bonds, local labels (tile labeling + merge inside the slab), edge record
+ *     all-gather of the ranks' edge records (caller: NCCL / any transport), in rank order
+ *     xy_slab_flip    (every rank)  replicated union-find over the cut roots, overrides, coins by canonical root, flip
+ *     exchange of first rows -> halo rows (caller), before the next xy_slab_label or xy_measure.
+ * xy_measure / xy_get_series return the slab's PARTIAL sums (its sites; the y links of its last row use the halo row;
+ * n_clusters counts the clusters whose canonical root lies in the slab): the caller adds the ranks' records.
+ * xy_get_labels returns canonical labels of the whole lattice (after xy_slab_flip).  xy_sw_sweeps, xy_pcc_run,
+ * xy_label_bonds and xy_debug_check_labels return XY_ERR_STATE on a slab. */
+int xy_slab_workspace_bytes(uint32_t L, uint32_t rows, uint32_t flags, size_t *nbytes);
+int xy_slab_create(xy_state **out, uint32_t L, uint32_t rows, uint32_t y_off, uint64_t seed, int init, uint32_t flags,
+                   void *dev_workspace, size_t nbytes);      /* dev_workspace NULL: the library allocates */
+/* device pointers (inside the workspace) of the buffers the caller exchanges: the slab's first row (send), its halo
+ * row (receive: row_bytes = 4 L), and its edge record (send: edge_bytes; layout: u64 root of every site of the first
+ * row, u64 root of every site of the last row, as site indices of the whole lattice, then one byte per site of the
+ * last row: its +y bond) */
+int xy_slab_buffers(xy_state *s, void **dev_first_row, void **dev_halo_row, size_t *row_bytes, void **dev_edges, size_t *edge_bytes);
+int xy_slab_label(xy_state *s, double beta, void *cuda_stream);
+/* dev_gathered_edges: nranks edge records in rank order (device memory) */
+int xy_slab_flip(xy_state *s, const void *dev_gathered_edges, uint32_t nranks, uint32_t rank, void *cuda_stream);
+
 /* ---- q-state Potts model on the same labeling core ------------------------
  * PAPER.md:30-34 cites the authors' GPU Swendsen-Wang codes for the Potts and Ising models (refs 19, 22)
  * as the origin of the labeling method; the update rule is not restated there and is the textbook one

@@ -107,6 +107,11 @@ _SIGS = {
     "xy_get_launch_count": [_vp, C.POINTER(C.c_uint64)],
     "xy_label_bonds": [_vp, _vp, C.c_size_t],
     "xy_debug_check_counts": [C.POINTER(C.c_uint64), C.POINTER(C.c_int)],
+    "xy_slab_workspace_bytes": [C.c_uint32, C.c_uint32, C.c_uint32, C.POINTER(C.c_size_t)],
+    "xy_slab_create": [C.POINTER(_vp), C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint64, C.c_int, C.c_uint32, _vp, C.c_size_t],
+    "xy_slab_buffers": [_vp, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(C.c_size_t), C.POINTER(_vp), C.POINTER(C.c_size_t)],
+    "xy_slab_label": [_vp, C.c_double, _vp],
+    "xy_slab_flip": [_vp, _vp, C.c_uint32, C.c_uint32, _vp],
     "xy_potts_create": [C.POINTER(_vp), C.c_uint32, C.c_uint32, C.c_uint64, C.c_int],
     "xy_potts_destroy": [_vp],
     "xy_potts_sweeps": [_vp, C.c_double, C.c_uint64, _vp],
@@ -319,6 +324,44 @@ def debug_philox(ctr, key):
 
 def debug_curand_philox(ctr, key):
     return _philox_common(_lib.xy_debug_curand_philox, ctr, key)
+
+
+# ---------------------------------------------------------------------------------------------
+# Row slab of a sharded lattice (include/xy.h, section "row-slab sharding"); the exchange between xy_slab_label and
+# xy_slab_flip is the caller's: paper_1210_6116_b200/shard.py does it with torch.distributed
+# ---------------------------------------------------------------------------------------------
+class SlabState(XYState):
+    """rows [y_off, y_off + rows) of an L x L lattice on the current CUDA device (marshalling only)."""
+
+    def __init__(self, L, rows, y_off, seed, init=INIT_HOT, flags=0):
+        import torch
+        if not torch.cuda.is_available():
+            raise XYError(-4, "no CUDA device: this library has no CPU fallback")
+        self.L, self.rows, self.y_off, self.N, self.seed, self.flags = L, rows, y_off, rows * L, seed, flags
+        self._h = _vp()
+        n = C.c_size_t()
+        _check(_lib.xy_slab_workspace_bytes(L, rows, flags, C.byref(n)))
+        self._ws = torch.empty(n.value, dtype=torch.uint8, device="cuda")
+        _check(_lib.xy_slab_create(C.byref(self._h), L, rows, y_off, seed, init, flags, self._ws.data_ptr(), n.value))
+        first, halo, edges = _vp(), _vp(), _vp()
+        rb, eb = C.c_size_t(), C.c_size_t()
+        _check(_lib.xy_slab_buffers(self._h, C.byref(first), C.byref(halo), C.byref(rb), C.byref(edges), C.byref(eb)))
+        base = self._ws.data_ptr()
+        # views into the workspace tensor (the exchange reads / writes them in place)
+        self.first_row = self._ws[first.value - base: first.value - base + rb.value].view(torch.float32)
+        self.halo_row = self._ws[halo.value - base: halo.value - base + rb.value].view(torch.float32)
+        self.edges = self._ws[edges.value - base: edges.value - base + eb.value]
+
+    def slab_label(self, beta, stream=None):
+        import torch
+        st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+        _check(_lib.xy_slab_label(self._h, beta, st))
+
+    def slab_flip(self, gathered, nranks, rank, stream=None):
+        import torch
+        st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+        assert gathered.is_cuda and gathered.is_contiguous() and gathered.numel() * gathered.element_size() == nranks * self.edges.numel()
+        _check(_lib.xy_slab_flip(self._h, gathered.data_ptr(), nranks, rank, st))
 
 
 # ---------------------------------------------------------------------------------------------

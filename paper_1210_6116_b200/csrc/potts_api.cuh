@@ -37,6 +37,7 @@ SweepArgs potts_sweep_args(const xy_potts *s)
     a.bonds = s->bonds();
     a.rootmask = s->rootmask();
     a.L = s->L;
+    a.rows = s->L;
     a.tiles_x = s->L / s->ker.tw;
     a.ntiles = a.tiles_x * (s->L / s->ker.th);
     set_Ldiv(a, s->L);

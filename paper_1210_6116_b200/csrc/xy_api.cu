@@ -3,6 +3,7 @@
 // phi_t from the host-side Philox, the reflection constant), launch sequencing, ring bookkeeping.
 // Every step of the hot path runs in the kernels of xy_kernels.cuh; there is no CPU fallback.
 #include "xy_kernels.cuh"
+#include "slab_kernels.cuh"
 
 #include <curand_philox4x32_x.h>   // NVIDIA's curand_Philox4x32_10, for xy_debug_curand_philox only
 
@@ -45,16 +46,19 @@ constexpr size_t kStageBytes = 64u << 20;  // staging buffer of the debug getter
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-    size_t theta, labels, bonds, rootmask, partials, ring, fring, ctl, tab, total;
+    size_t theta, labels, bonds, rootmask, partials, ring, fring, ctl, tab, edges, xroot, total;
 };
 
-Layout make_layout(uint32_t L, uint32_t flags)
+// rows == L and slab == false: a whole lattice.  A slab holds `rows` rows plus one halo row of
+// theta, its edge record for the all-gather and the table of overridden roots.
+Layout make_layout(uint32_t L, uint32_t flags, uint32_t rows = 0, bool slab = false)
 {
-    const size_t N = (size_t)L * L;
+    if (rows == 0) rows = L;
+    const size_t N = (size_t)rows * L;
     const size_t lw = (flags & XY_FLAG_LABELS64) ? 8 : 4;
     Layout o;
     size_t off = 0;
-    o.theta = off;    off = align_up(off + N * 4, 256);
+    o.theta = off;    off = align_up(off + (N + (slab ? L : 0)) * 4, 256);
     o.labels = off;   off = align_up(off + N * lw, 256);
     o.bonds = off;    off = align_up(off + N / 4, 256);
     o.rootmask = off; off = align_up(off + N / 8, 256);
@@ -63,6 +67,8 @@ Layout make_layout(uint32_t L, uint32_t flags)
     o.fring = off;    off = align_up(off + ((flags & XY_FLAG_FOURIER) ? (size_t)kRingCap * sizeof(xy_fourier) : 0), 256);
     o.ctl = off;      off = align_up(off + sizeof(DevCtl), 256);
     o.tab = off;      off = align_up(off + (size_t)(kTabN + 1) * sizeof(double2), 256);
+    o.edges = off;    off = align_up(off + (slab ? slab_edge_bytes(L) : 0), 256);
+    o.xroot = off;    off = align_up(off + (slab ? (size_t)2 * L * 8 : 0), 256);
     o.total = off;
     return o;
 }
@@ -74,6 +80,7 @@ struct Kernels {
     void (*label)(const SweepArgs &, cudaStream_t);
     void (*merge)(const SweepArgs &, cudaStream_t);
     void (*flip)(const SweepArgs &, int grid, cudaStream_t);
+    void (*flip_slab)(const SweepArgs &, cudaStream_t);
     int (*prepare)(bool fourier, int *bonds_obs, int *bonds_noobs, int *fl);
     int tw, th, rs;
 };
@@ -90,8 +97,18 @@ struct KS {
         k_bonds<VEC, RS, kB, kO, kF><<<grid, BondsShape<kO>::warps * 32, k_bonds_smem_bytes<kO>(), st>>>(a);
         return cudaGetLastError();
     }
+    template <bool kB, bool kO>
+    static cudaError_t bonds_slab_launch(const SweepArgs &a, int grid, cudaStream_t st)
+    {
+        k_bonds<VEC, RS, kB, kO, false, true><<<grid, BondsShape<kO>::warps * 32, k_bonds_smem_bytes<kO>(), st>>>(a);
+        return cudaGetLastError();
+    }
     static cudaError_t bonds(const SweepArgs &a, int what, bool fourier, int grid, cudaStream_t st)
     {
+        if (a.open_y) {
+            if (what == 2) return bonds_slab_launch<true, false>(a, grid, st);
+            return what == 1 ? bonds_slab_launch<false, true>(a, grid, st) : bonds_slab_launch<true, true>(a, grid, st);
+        }
         if (what == 2) return bonds_launch<true, false, false>(a, grid, st);
         if (fourier) return what == 1 ? bonds_launch<false, true, true>(a, grid, st) : bonds_launch<true, true, true>(a, grid, st);
         return what == 1 ? bonds_launch<false, true, false>(a, grid, st) : bonds_launch<true, true, false>(a, grid, st);
@@ -111,6 +128,10 @@ struct KS {
     {
         (void)grid;
         k_flip<VEC, R * NW, LabelT><<<a.ntiles, VEC * R * NW, 0, st>>>(a);
+    }
+    static void flip_slab(const SweepArgs &a, cudaStream_t st)
+    {
+        if constexpr (sizeof(LabelT) == 4) k_flip<VEC, R * NW, LabelT, true><<<a.ntiles, VEC * R * NW, 0, st>>>(a);
     }
     template <bool kB, bool kO, bool kF>
     static cudaError_t bonds_prepare(int *occ)
@@ -139,6 +160,10 @@ struct KS {
             if (e == cudaSuccess) e = bonds_prepare<false, true, false>(bonds_obs);
         }
         if (e == cudaSuccess) e = bonds_prepare<true, false, false>(bonds_noobs);
+        // the slab variants: same shapes and shared memory
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bonds<VEC, RS, true, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k_bonds_smem_bytes<true>());
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bonds<VEC, RS, false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k_bonds_smem_bytes<true>());
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_bonds<VEC, RS, true, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k_bonds_smem_bytes<false>());
         if (e == cudaSuccess)
             e = cudaFuncSetAttribute(k_label<VEC, R * NW, LabelT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      (int)k_label_smem_bytes<VEC, R * NW>());
@@ -147,7 +172,7 @@ struct KS {
     }
     static Kernels get()
     {
-        return Kernels{&bonds, &label, &merge, &flip, &prepare, 32 * VEC, R * NW, RS};
+        return Kernels{&bonds, &label, &merge, &flip, &flip_slab, &prepare, 32 * VEC, R * NW, RS};
     }
 };
 
@@ -234,7 +259,13 @@ __global__ void k_pcc_setup(DevCtl *c, PccSetup s)
 
 struct xy_state {
     uint32_t L = 0, flags = 0;
-    uint64_t N = 0, seed = 0;
+    uint32_t rows = 0, y_off = 0;   // the state holds rows [y_off, y_off + rows) of the L x L lattice (rows == L: all of it)
+    bool slab = false;              // created by xy_slab_create: open in y, halo row, stitch
+    bool slab_labelled = false;     // xy_slab_label done, xy_slab_flip pending
+    StitchTable stitch{};           // replicated union-find over the cut roots (device memory, allocated at the first flip)
+    uint32_t stitch_ranks = 0;
+    SweepArgs pending{};            // arguments of the sweep between xy_slab_label and xy_slab_flip
+    uint64_t N = 0, seed = 0;       // N: sites held by this state
     uint64_t T = 0;                 // sweeps done
     int device = 0;
     bool owns_ws = false;
@@ -268,6 +299,8 @@ struct xy_state {
     xy_obs *ring() const { return reinterpret_cast<xy_obs *>(ws + lay.ring); }
     DevCtl *ctl() const { return reinterpret_cast<DevCtl *>(ws + lay.ctl); }
     double2 *tab() const { return reinterpret_cast<double2 *>(ws + lay.tab); }
+    unsigned char *edges() const { return reinterpret_cast<unsigned char *>(ws + lay.edges); }
+    uint64_t *xroot() const { return reinterpret_cast<uint64_t *>(ws + lay.xroot); }
     bool l64() const { return (flags & XY_FLAG_LABELS64) != 0; }
     bool fourier() const { return (flags & XY_FLAG_FOURIER) != 0; }
     xy_fourier *fring() const { return reinterpret_cast<xy_fourier *>(ws + lay.fring); }
@@ -313,7 +346,11 @@ SweepArgs base_args(const xy_state *s)
     a.ring_cap = kRingCap;
     a.L = s->L;
     a.tiles_x = s->L / s->ker.tw;
-    a.ntiles = a.tiles_x * (s->L / s->ker.th);
+    a.ntiles = a.tiles_x * (s->rows / s->ker.th);
+    a.rows = s->rows;
+    a.y_off = s->y_off;
+    a.open_y = s->slab ? 1 : 0;
+    a.xroot = s->xroot();
     set_Ldiv(a, s->L);
     a.seed_lo = (uint32_t)(s->seed & 0xffffffffu);
     a.seed_hi = (uint32_t)(s->seed >> 32);
@@ -453,26 +490,39 @@ int xy_workspace_bytes(uint32_t L, uint32_t flags, size_t *nbytes)
     return XY_OK;
 }
 
-int xy_create_ex(xy_state **out, uint32_t L, uint64_t seed, int init, uint32_t flags, void *dev_workspace, size_t nbytes)
+static int check_slab(uint32_t L, uint32_t rows, uint32_t y_off, uint32_t flags)
+{
+    if (rows < 32 || rows % 32 != 0 || y_off % 32 != 0 || (uint64_t)y_off + rows > L)
+        return fail(XY_ERR_ARG, "slab rows [%u, %u + %u) must be multiples of 32 inside 0..%u", y_off, y_off, rows, L);
+    if ((uint64_t)rows * L >= 0x80000000ull) return fail(XY_ERR_ARG, "a slab holds fewer than 2^31 sites (u32 labels with one flag bit)");
+    if (flags & XY_FLAG_LABELS64) return fail(XY_ERR_ARG, "slabs use 32-bit labels");
+    if (flags & XY_FLAG_FOURIER) return fail(XY_ERR_ARG, "slabs do not reduce the structure-factor sums");
+    return XY_OK;
+}
+
+static int create_common(xy_state **out, uint32_t L, uint32_t rows, uint32_t y_off, bool slab, uint64_t seed, int init,
+                         uint32_t flags, void *dev_workspace, size_t nbytes)
 {
     if (!out) return fail(XY_ERR_ARG, "out is NULL");
     *out = nullptr;
     if (int rc = check_L(L)) return rc;
     if (init != XY_INIT_COLD && init != XY_INIT_HOT) return fail(XY_ERR_ARG, "init=%d unknown", init);
     if (flags & ~(uint32_t)(XY_FLAG_LABELS64 | XY_FLAG_FOURIER)) return fail(XY_ERR_ARG, "unknown flags 0x%x", flags);
+    if (slab) if (int rc = check_slab(L, rows, y_off, flags)) return rc;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
         return fail(XY_ERR_CUDA, "no CUDA device: this library has no CPU fallback");
     xy_state *s = new (std::nothrow) xy_state;
     if (!s) return fail(XY_ERR_NOMEM, "host allocation failed");
-    s->L = L; s->N = (uint64_t)L * L; s->seed = seed; s->flags = flags;
-    s->lay = make_layout(L, flags);
+    s->L = L; s->rows = rows; s->y_off = y_off; s->slab = slab;
+    s->N = (uint64_t)rows * L; s->seed = seed; s->flags = flags;
+    s->lay = make_layout(L, flags, rows, slab);
     s->ker = pick_kernels(L, s->l64());
     cudaGetDevice(&s->device);
     if (dev_workspace) {
         if (nbytes < s->lay.total || ((uintptr_t)dev_workspace & 255u)) {
             delete s;
-            return fail(XY_ERR_ARG, "workspace too small (%zu < %zu) or not 256-byte aligned", nbytes, make_layout(L, flags).total);
+            return fail(XY_ERR_ARG, "workspace too small (%zu < %zu) or not 256-byte aligned", nbytes, make_layout(L, flags, rows, slab).total);
         }
         s->ws = static_cast<char *>(dev_workspace);
     } else {
@@ -496,8 +546,8 @@ int xy_create_ex(xy_state **out, uint32_t L, uint64_t seed, int init, uint32_t f
         return fail(XY_ERR_CUDA, "kernel occupancy query failed: %s (was the library built for this GPU's sm_100a?)",
                     cudaGetErrorString(e));
     }
-    const uint32_t ntiles = (L / s->ker.tw) * (L / s->ker.th);
-    const uint32_t nstrips = (L / s->ker.tw) * (L / s->ker.rs);
+    const uint32_t ntiles = (L / s->ker.tw) * (rows / s->ker.th);
+    const uint32_t nstrips = (L / s->ker.tw) * (rows / s->ker.rs);
     // the variants of k_bonds with observables share ONE grid so that their fixed-order sums agree bitwise
     long need = (nstrips + BondsShape<true>::warps - 1) / BondsShape<true>::warps;
     long g = (long)sms * bo;
@@ -531,9 +581,9 @@ int xy_create_ex(xy_state **out, uint32_t L, uint64_t seed, int init, uint32_t f
     }
 
     if (init == XY_INIT_COLD) {
-        e = cudaMemsetAsync(s->theta(), 0, s->N * 4, nullptr);
+        e = cudaMemsetAsync(s->theta(), 0, (s->N + (slab ? L : 0)) * 4, nullptr);
     } else {
-        k_init_hot<<<148 * 8, 256>>>(s->theta(), s->N, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32));
+        k_init_hot<<<148 * 8, 256>>>(s->theta(), s->N, (uint64_t)y_off * L, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32));
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) {
@@ -550,6 +600,11 @@ int xy_create_ex(xy_state **out, uint32_t L, uint64_t seed, int init, uint32_t f
     return XY_OK;
 }
 
+int xy_create_ex(xy_state **out, uint32_t L, uint64_t seed, int init, uint32_t flags, void *dev_workspace, size_t nbytes)
+{
+    return create_common(out, L, L, 0, false, seed, init, flags, dev_workspace, nbytes);
+}
+
 int xy_create(xy_state **out, uint32_t L, uint64_t seed, int init)
 {
     return xy_create_ex(out, L, seed, init, 0, nullptr, 0);
@@ -562,6 +617,7 @@ int xy_destroy(xy_state *s)
     cudaStreamSynchronize(s->stream);
     for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
     if (s->stage) cudaFree(s->stage);
+    if (s->stitch.key) cudaFree(s->stitch.key);
     if (s->owns_ws) cudaFree(s->ws);
     delete s;
     return XY_OK;
@@ -598,6 +654,7 @@ int xy_sw_sweeps(xy_state *s, double beta, uint64_t n, void *cuda_stream)
     if (!s) return fail(XY_ERR_ARG, "state is NULL");
     if (!(beta >= 0.0) || !std::isfinite(beta)) return fail(XY_ERR_ARG, "beta must be finite and >= 0");
     if (s->T + n > 0xffffffffull) return fail(XY_ERR_STATE, "sweep counter would reach 2^32");
+    if (s->slab) return fail(XY_ERR_STATE, "a slab sweeps with xy_slab_label / xy_slab_flip (an exchange lies between them)");
     DeviceGuard g(s->device);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     if (st != s->stream) {
@@ -628,6 +685,7 @@ int xy_pcc_run(xy_state *s, double beta0, double dbeta0, const xy_pcc_schedule *
     if (sc->window < 1 || (sc->dirs != 1 && sc->dirs != 2)) return fail(XY_ERR_ARG, "window must be >= 1 and dirs 1 or 2");
     if (sc->discard > sc->n_sweeps) return fail(XY_ERR_ARG, "discard > n_sweeps");
     if (s->T + sc->n_sweeps > 0xffffffffull) return fail(XY_ERR_STATE, "sweep counter would reach 2^32");
+    if (s->slab) return fail(XY_ERR_STATE, "the PCC controller needs the sums of the whole lattice: not available on a slab");
     DeviceGuard g(s->device);
     const uint64_t measured = sc->n_sweeps - sc->discard;
     const uint64_t max_dec = measured / sc->window;
@@ -868,6 +926,19 @@ int xy_get_labels_range(xy_state *s, int64_t *host, uint64_t first, size_t n)
     if (!s->have_sweep) return fail(XY_ERR_STATE, "no sweep has produced labels yet");
     DeviceGuard g(s->device);
     if (int rc = ensure_stage(s)) return rc;
+    if (s->slab) {
+        // canonical labels of the whole lattice; valid after xy_slab_flip (the stitch overrides are in place)
+        if (s->slab_labelled) return fail(XY_ERR_STATE, "labels of a slab are complete after xy_slab_flip");
+        const uint64_t chunk = kStageBytes / sizeof(int64_t);
+        for (uint64_t done = 0; done < n; done += chunk) {
+            const uint64_t m = n - done < chunk ? n - done : chunk;
+            k_slab_labels_to_i64<<<148 * 4, 256, 0, s->stream>>>(static_cast<const uint32_t *>(s->labels()), s->xroot(),
+                                                                 (uint64_t)s->y_off * s->L, static_cast<int64_t *>(s->stage), first + done, m);
+            CUDA_TRY(cudaMemcpyAsync(host + done, s->stage, m * sizeof(int64_t), cudaMemcpyDeviceToHost, s->stream));
+            CUDA_TRY(cudaStreamSynchronize(s->stream));
+        }
+        return XY_OK;
+    }
     if (int rc = ensure_flat(s)) return rc;
     const uint64_t chunk = kStageBytes / sizeof(int64_t);
     for (uint64_t done = 0; done < n; done += chunk) {
@@ -886,6 +957,7 @@ int xy_debug_check_labels(xy_state *s, uint64_t counts[5])
 {
     if (!s || !counts) return fail(XY_ERR_ARG, "NULL argument");
     if (!s->have_sweep) return fail(XY_ERR_STATE, "no sweep has produced labels yet");
+    if (s->slab) return fail(XY_ERR_STATE, "not available on a slab");
     DeviceGuard g(s->device);
     if (int rc = ensure_stage(s)) return rc;
     if (int rc = ensure_flat(s)) return rc;
@@ -925,6 +997,7 @@ int xy_label_bonds(xy_state *s, const uint8_t *host_bonds, size_t n)
 {
     if (!s || !host_bonds) return fail(XY_ERR_ARG, "NULL argument");
     if (n != s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
+    if (s->slab) return fail(XY_ERR_STATE, "not available on a slab");
     DeviceGuard g(s->device);
     if (int rc = ensure_stage(s)) return rc;
     const uint64_t chunk = kStageBytes;            // canonical bytes per pass (multiple of 4)
@@ -979,6 +1052,113 @@ static int debug_philox_common(const uint32_t *ctr, const uint32_t *key, uint32_
     if (e == cudaSuccess) e = cudaMemcpy(out, d + 6 * n, n * 16, cudaMemcpyDeviceToHost);
     cudaFree(d);
     if (e != cudaSuccess) return fail(XY_ERR_CUDA, "debug philox failed: %s", cudaGetErrorString(e));
+    return XY_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Row-slab sharding: one state per rank holds rows [y_off, y_off + rows).
+// ---------------------------------------------------------------------------------------------
+int xy_slab_workspace_bytes(uint32_t L, uint32_t rows, uint32_t flags, size_t *nbytes)
+{
+    if (!nbytes) return fail(XY_ERR_ARG, "nbytes is NULL");
+    if (int rc = check_L(L)) return rc;
+    if (flags & ~(uint32_t)(XY_FLAG_LABELS64 | XY_FLAG_FOURIER)) return fail(XY_ERR_ARG, "unknown flags 0x%x", flags);
+    if (int rc = check_slab(L, rows, 0, flags)) return rc;
+    *nbytes = make_layout(L, flags, rows, true).total;
+    return XY_OK;
+}
+
+int xy_slab_create(xy_state **out, uint32_t L, uint32_t rows, uint32_t y_off, uint64_t seed, int init, uint32_t flags,
+                   void *dev_workspace, size_t nbytes)
+{
+    return create_common(out, L, rows, y_off, true, seed, init, flags, dev_workspace, nbytes);
+}
+
+int xy_slab_buffers(xy_state *s, void **dev_first_row, void **dev_halo_row, size_t *row_bytes, void **dev_edges, size_t *edge_bytes)
+{
+    if (!s || !dev_first_row || !dev_halo_row || !row_bytes || !dev_edges || !edge_bytes) return fail(XY_ERR_ARG, "NULL argument");
+    if (!s->slab) return fail(XY_ERR_STATE, "not a slab");
+    *dev_first_row = s->theta();
+    *dev_halo_row = s->theta() + s->N;
+    *row_bytes = (size_t)s->L * sizeof(float);
+    *dev_edges = s->edges();
+    *edge_bytes = slab_edge_bytes(s->L);
+    return XY_OK;
+}
+
+int xy_slab_label(xy_state *s, double beta, void *cuda_stream)
+{
+    if (!s) return fail(XY_ERR_ARG, "state is NULL");
+    if (!s->slab) return fail(XY_ERR_STATE, "not a slab");
+    if (s->slab_labelled) return fail(XY_ERR_STATE, "xy_slab_flip of the previous xy_slab_label is pending");
+    if (!(beta >= 0.0) || !std::isfinite(beta)) return fail(XY_ERR_ARG, "beta must be finite and >= 0");
+    if (s->T >= 0xffffffffull) return fail(XY_ERR_STATE, "sweep counter would reach 2^32");
+    DeviceGuard g(s->device);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (st != s->stream) {
+        CUDA_TRY(cudaStreamSynchronize(s->stream));
+        s->stream = st;
+    }
+    SweepArgs a = base_args(s);
+    set_direction(s, s->T, a);
+    a.beta = beta;
+    const bool with_obs = s->obs_mode == XY_OBS_ALL && s->obs_valid_T != s->T;
+    a.obs_fill = with_obs ? 1 : 0;
+    if (with_obs) CUDA_TRY(s->ker.bonds(a, 0, s->fourier(), s->grid_bonds, s->stream));
+    else CUDA_TRY(s->ker.bonds(a, 2, false, s->grid_bonds_noobs, s->stream));
+    s->ker.label(a, s->stream);
+    s->ker.merge(a, s->stream);
+    k_slab_edges<<<(s->L + 255) / 256, 256, 0, s->stream>>>(static_cast<const uint32_t *>(s->labels()), s->bonds(), s->L,
+                                                           s->rows, s->y_off, s->edges());
+    CUDA_TRY(cudaGetLastError());
+    s->launches += 4;
+    if (a.obs_fill) s->obs_valid_T = s->T;
+    s->pending = a;
+    s->slab_labelled = true;
+    return XY_OK;
+}
+
+int xy_slab_flip(xy_state *s, const void *dev_gathered_edges, uint32_t nranks, uint32_t rank, void *cuda_stream)
+{
+    if (!s || !dev_gathered_edges) return fail(XY_ERR_ARG, "NULL argument");
+    if (!s->slab) return fail(XY_ERR_STATE, "not a slab");
+    if (!s->slab_labelled) return fail(XY_ERR_STATE, "call xy_slab_label first");
+    if (nranks < 1 || rank >= nranks) return fail(XY_ERR_ARG, "rank %u of %u", rank, nranks);
+    DeviceGuard g(s->device);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (st != s->stream) {
+        CUDA_TRY(cudaStreamSynchronize(s->stream));
+        s->stream = st;
+    }
+    const uint64_t entries = (uint64_t)nranks * 2u * s->L;
+    if (entries >= (1ull << 29)) return fail(XY_ERR_ARG, "too many cut sites");
+    if (s->stitch_ranks != nranks) {
+        if (s->stitch.key) { CUDA_TRY(cudaStreamSynchronize(s->stream)); cudaFree(s->stitch.key); s->stitch = StitchTable{}; }
+        uint32_t cap = 1024;
+        while (cap < 4 * entries) cap <<= 1;
+        void *p = nullptr;
+        CUDA_TRY(cudaMalloc(&p, (size_t)cap * 12 + entries * 4));
+        s->stitch.key = static_cast<uint64_t *>(p);
+        s->stitch.parent = reinterpret_cast<uint32_t *>(s->stitch.key + cap);
+        s->stitch.slot_of = s->stitch.parent + cap;
+        s->stitch.cap_mask = cap - 1;
+        s->stitch_ranks = nranks;
+    }
+    const unsigned char *gathered = static_cast<const unsigned char *>(dev_gathered_edges);
+    const int grid = 148 * 4;
+    k_stitch_clear<<<grid, 256, 0, s->stream>>>(s->stitch);
+    k_stitch_insert<<<grid, 256, 0, s->stream>>>(s->stitch, gathered, s->L, nranks);
+    k_stitch_union<<<grid, 256, 0, s->stream>>>(s->stitch, gathered, s->L, nranks);
+    k_stitch_apply<<<(2 * s->L + 255) / 256, 256, 0, s->stream>>>(s->stitch, gathered, s->L, rank, s->y_off,
+                                                                 static_cast<uint32_t *>(s->labels()), s->xroot());
+    s->ker.flip_slab(s->pending, s->stream);
+    CUDA_TRY(cudaGetLastError());
+    s->launches += 5;
+    s->slab_labelled = false;
+    s->T += 1;
+    if (s->T - s->oldest_T >= kRingCap) s->oldest_T = s->T - kRingCap + 1;
+    s->have_sweep = true;
+    s->labels_flat = false;
     return XY_OK;
 }
 

@@ -92,12 +92,13 @@ __device__ __noinline__ bool bond_exact(float ti, float tj, double phi, double b
 
 // The same for the bond of site (y, x) in direction dir (0: +x, 1: +y), angles re-read from memory
 // (the streaming loop does not keep them once (cos, sin, sigma) are evaluated).
-__device__ __noinline__ bool bond_exact_at(const float *theta, uint32_t L, uint32_t y, uint32_t x, int dir,
+// wrap_rows: number of rows after which y wraps to row 0 (0: never: a slab, whose row below the last is its halo row)
+__device__ __noinline__ bool bond_exact_at(const float *theta, uint32_t L, uint32_t wrap_rows, uint32_t y, uint32_t x, int dir,
                                            double phi, double beta, uint32_t w, unsigned long long *fallback_counter)
 {
     uint32_t x2 = x, y2 = y;
     if (dir == 0) { x2 = x + 1; if (x2 == L) x2 = 0; }
-    else { y2 = y + 1; if (y2 == L) y2 = 0; }
+    else { y2 = y + 1; if (y2 == wrap_rows) y2 = 0; }
     return bond_exact(theta[(size_t)y * L + x], theta[(size_t)y2 * L + x2], phi, beta, w, fallback_counter);
 }
 

@@ -70,7 +70,17 @@ struct SweepArgs {
     const double2 *sincos_tab;    // [kTabN + 1] (cos, sin)(k / 1024), host-computed
     double       ck1, sk1;        // (cos, sin)(2 pi / L)
     xy_fourier  *fring;           // ring of structure-factor records (XY_FLAG_FOURIER), else unused
+    // slab of a lattice sharded by rows: the state holds rows [y_off, y_off + rows) of the
+    // L x L lattice; rows == L, y_off == 0, open_y == 0 for a whole lattice
+    uint32_t     rows, y_off;
+    int          open_y;          // 1: no periodic wrap in y: row `rows` of theta is the halo row (the neighbour's first
+                                  //    row), the y bonds of the last row are left to the stitch
+    const uint64_t *xroot;        // slab: global canonical roots of the local roots the stitch overrode (k_flip)
 };
+
+// slab mode: label[r] of a local root r whose cluster reaches into another slab and has its canonical root there is
+// kSlabSpecial | k: its global root is xroot[k] (labels are u32 words in slab mode, local indices below 2^31)
+constexpr uint32_t kSlabSpecial = 0x80000000u;
 
 
 template <int VEC> struct FVec;
@@ -212,7 +222,7 @@ __device__ __forceinline__ void site_eval(float theta, uint32_t tab_adj, float &
 template <int VEC> struct RowSigma { float pg[VEC], g[VEC], gn; };
 
 template <int VEC>
-__device__ __noinline__ uint32_t bonds_fix(const float *theta, uint32_t L, uint32_t seed_lo, uint32_t seed_hi, uint32_t t,
+__device__ __noinline__ uint32_t bonds_fix(const float *theta, uint32_t L, uint32_t wrap_rows, uint32_t seed_lo, uint32_t seed_hi, uint32_t t,
                                            BondCtx bcx, uint64_t quad, uint32_t gy, uint32_t xl, RowSigma<VEC> rs, uint32_t bits)
 {
     const U4 wA = rng(seed_lo, seed_hi, quad, t, TAG_BOND);
@@ -235,21 +245,24 @@ __device__ __noinline__ uint32_t bonds_fix(const float *theta, uint32_t L, uint3
         if (!(fabsf(dx) > bcx.delta)) {
             const uint32_t wx = (wa[v] << 16) | (wb[v] & 0xffffu);
             bits &= ~(1u << v);
-            if (bond_exact_at(theta, L, gy, xl + v, 0, bcx.phi, bcx.beta, wx, bcx.fallback_counter)) bits |= 1u << v;
+            if (bond_exact_at(theta, L, wrap_rows, gy, xl + v, 0, bcx.phi, bcx.beta, wx, bcx.fallback_counter)) bits |= 1u << v;
         }
         if (!(fabsf(dy) > bcx.delta)) {
             const uint32_t wy = (wa[v] & 0xffff0000u) | (wb[v] >> 16);
             bits &= ~(0x100u << v);
-            if (bond_exact_at(theta, L, gy, xl + v, 1, bcx.phi, bcx.beta, wy, bcx.fallback_counter)) bits |= 0x100u << v;
+            if (bond_exact_at(theta, L, wrap_rows, gy, xl + v, 1, bcx.phi, bcx.beta, wy, bcx.fallback_counter)) bits |= 0x100u << v;
         }
     }
     return bits;
 }
 
-template <int VEC, int RS, bool kBonds, bool kObs, bool kFourier>
+// kSlab: the state is a slab of rows of a sharded lattice: `rows` rows, no wrap in y (row `rows`
+// of theta is the halo row), quad indices (Philox counters) of the whole lattice.
+template <int VEC, int RS, bool kBonds, bool kObs, bool kFourier, bool kSlab = false>
 __global__ void __launch_bounds__(BondsShape<kObs>::warps * 32, BondsShape<kObs>::min_ctas)
 k_bonds(const SweepArgs a)
 {
+    static_assert(!(kSlab && kFourier), "slabs do not reduce the structure-factor sums");
     static_assert(kObs || !kFourier, "the structure-factor sums are observables");
     static_assert(kBonds || kObs, "nothing to do");
     constexpr int NW = BondsShape<kObs>::warps;
@@ -295,7 +308,10 @@ k_bonds(const SweepArgs a)
     uint32_t nbx = 0, nby = 0;
 
     const uint32_t strips_x = L / TW;
-    const uint32_t nstrips = strips_x * (L / RS);
+    const uint32_t nstrips = strips_x * ((kSlab ? a.rows : L) / RS);
+    // slab: the quad index (Philox counter) is that of the whole lattice; the bond bytes are addressed with it from a
+    // base moved back by the slab's first quad
+    uint8_t *const bonds_g = kSlab ? a.bonds - (((uint64_t)a.y_off * L) >> 2) : a.bonds;
     for (uint32_t strip = blockIdx.x * NW + warp; strip < nstrips; strip += gridDim.x * NW) {
         const uint32_t sy = strip / strips_x, sx = strip - sy * strips_x;
         const uint32_t y0 = sy * RS;
@@ -330,9 +346,9 @@ k_bonds(const SweepArgs a)
         // running addresses (one 64-bit add per row each): quad index of the lane's first site in the row
         // being finished (Philox counter, bond byte), and the row to load next; only the y-halo row of the
         // lattice's last strip row wraps
-        uint64_t quad = ((uint64_t)y0 * L + xl) >> 2;
+        uint64_t quad = ((uint64_t)((kSlab ? a.y_off : 0u) + y0) * L + xl) >> 2;
         const float *nxt = a.theta + (size_t)y0 * L + xl;
-        const float *halo_row = a.theta + (y0 + RS == L ? (size_t)0 : (size_t)(y0 + RS) * L) + xl;
+        const float *halo_row = a.theta + (!kSlab && y0 + RS == L ? (size_t)0 : (size_t)(y0 + RS) * L) + xl;
         load_vec<VEC, true>(nxt, tA);
         nxt += L;
         load_vec<VEC, true>(RS == 1 ? halo_row : nxt, tB);
@@ -419,19 +435,19 @@ k_bonds(const SweepArgs a)
 #pragma unroll
                     for (int v = 0; v < VEC; ++v) { rsg.pg[v] = pg[v]; rsg.g[v] = g[v]; }
                     rsg.gn = gn;
-                    const uint32_t fixed = bonds_fix<VEC>(a.theta, L, a.seed_lo, a.seed_hi, a.t, bcx, quad, gy, xl, rsg, xn | (yn << 8));
+                    const uint32_t fixed = bonds_fix<VEC>(a.theta, L, kSlab ? 0u : L, a.seed_lo, a.seed_hi, a.t, bcx, quad, gy, xl, rsg, xn | (yn << 8));
                     xn = fixed & 0xffu;
                     yn = fixed >> 8;
                 }
                 nbx += __popc(xn);
                 nby += __popc(yn);
                 if constexpr (VEC == 4) {
-                    a.bonds[quad] = (uint8_t)(xn | (yn << 4));
+                    bonds_g[quad] = (uint8_t)(xn | (yn << 4));
                 } else {
                     // two lanes share a byte: even lane holds sites 4k,4k+1; odd lane 4k+2,4k+3
                     const uint32_t mine = xn | (yn << 4);
                     const uint32_t other = __shfl_xor_sync(0xffffffffu, mine, 1);
-                    if ((lane & 1) == 0) a.bonds[quad] = (uint8_t)(mine | (other << 2));
+                    if ((lane & 1) == 0) bonds_g[quad] = (uint8_t)(mine | (other << 2));
                 }
             }
             quad += L >> 2;
@@ -840,11 +856,12 @@ k_merge(const SweepArgs a)
                 bit = 3;                                   // bx of the 4th site of its byte
             } else {
                 x = tx * TW + (e - TH); y = ty * TH + TH - 1;
-                x2 = x; y2 = y + 1 == L ? 0 : y + 1;
+                x2 = x; y2 = y + 1 == a.rows ? 0 : y + 1;
                 bit = 4 + (x & 3u);
             }
             const size_t i = (size_t)y * L + x;
-            if ((a.bonds[i >> 2] >> bit) & 1u) {
+            const bool cut = a.open_y && e >= TH && y + 1 == a.rows;      // slab: that bond crosses into the next slab (stitch)
+            if (!cut && ((a.bonds[i >> 2] >> bit) & 1u)) {
                 active = true;
                 la = gload(labels + i);
                 lb = gload(labels + (size_t)y2 * L + x2);
@@ -871,8 +888,8 @@ k_merge(const SweepArgs a)
 //   sites   every other site reads the coin published by its tile root (its label), reflects,
 //           and rows in which nothing flipped are not written back.
 // ---------------------------------------------------------------------------------------------
-template <int WPR, int TH, typename LabelT>
-__global__ void __launch_bounds__(WPR * TH, (sizeof(LabelT) == 4 ? 1536 : 1024) / (WPR * TH))
+template <int WPR, int TH, typename LabelT, bool kSlab = false>
+__global__ void __launch_bounds__(WPR * TH, (sizeof(LabelT) == 4 && !kSlab ? 1536 : 1024) / (WPR * TH))
 k_flip(const SweepArgs a)
 {
     constexpr int TW = 32 * WPR, NT = WPR * TH;
@@ -903,8 +920,9 @@ k_flip(const SweepArgs a)
     asm volatile("cp.async.commit_group;" ::: "memory");
 
     if (tid == 0) nqueue = 0;
+    const uint64_t goff = kSlab ? (uint64_t)a.y_off * L : 0;      // slab: coins are keyed by the label in the whole lattice (a multiple of 128)
     if (tid < TH) {
-        const uint64_t g = (uint64_t)(y0 + tid) * L + x0;
+        const uint64_t g = (uint64_t)(y0 + tid) * L + x0 + goff;
         const U4 c = rng(a.seed_lo, a.seed_hi, g >> 7, a.t, TAG_FLIP);
         if constexpr (WPR == 4) {
             *reinterpret_cast<uint4 *>(&cbits[tid * 4]) = make_uint4(c.x, c.y, c.z, c.w);
@@ -943,7 +961,7 @@ k_flip(const SweepArgs a)
             if (lab[v] != (LabelT)(i + v)) merged |= 1u << (4 * k + v);
     }
     merged &= rb;
-    const uint32_t ncl = __popc(rb & ~merged);
+    uint32_t ncl = __popc(rb & ~merged);
     __syncthreads();                                 // nqueue = 0 and cbits visible
     while (merged) {
         const int b = __ffs(merged) - 1;
@@ -957,13 +975,31 @@ k_flip(const SweepArgs a)
         const uint32_t nq = nqueue;
         for (uint32_t j = tid; j < nq; j += NT) {
             const uint32_t loc = queue[j];
-            LabelT root = __ldg(labels + gbase + (LabelT)(loc / TW) * L + (loc % TW));
-            LabelT p = __ldg(labels + root);
-            while (p != root) { XY_CHECK(CHK_GLABEL, p < root); root = p; p = __ldg(labels + root); }
-            const U4 c = rng(a.seed_lo, a.seed_hi, (uint64_t)root >> 7, a.t, TAG_FLIP);
-            const uint32_t sel = ((uint32_t)root >> 5) & 3u;
+            const LabelT self = gbase + (LabelT)(loc / TW) * L + (loc % TW);
+            LabelT root = __ldg(labels + self);
+            uint64_t groot;                                  // canonical label in the whole lattice
+            if constexpr (kSlab) {
+                // slab: a chain may end in an entry the stitch overrode (kSlabSpecial | k): the root is xroot[k]
+                while (!((uint32_t)root & kSlabSpecial)) {
+                    const LabelT p = __ldg(labels + root);
+                    if (p == root) break;
+                    root = p;
+                }
+                if ((uint32_t)root & kSlabSpecial) {
+                    groot = a.xroot[(uint32_t)root & ~kSlabSpecial];
+                    if (groot == (uint64_t)self + goff) ++ncl;   // the cluster's canonical root is this very site
+                } else {
+                    groot = (uint64_t)root + goff;
+                }
+            } else {
+                LabelT p = __ldg(labels + root);
+                while (p != root) { XY_CHECK(CHK_GLABEL, p < root); root = p; p = __ldg(labels + root); }
+                groot = (uint64_t)root;
+            }
+            const U4 c = rng(a.seed_lo, a.seed_hi, groot >> 7, a.t, TAG_FLIP);
+            const uint32_t sel = ((uint32_t)groot >> 5) & 3u;
             const uint32_t word = sel == 0 ? c.x : sel == 1 ? c.y : sel == 2 ? c.z : c.w;
-            const uint32_t coin = (word >> ((uint32_t)root & 31u)) & 1u;
+            const uint32_t coin = (word >> ((uint32_t)groot & 31u)) & 1u;
             if (coin) atomicOr(&cbits[loc >> 5], 1u << (loc & 31u));
             else atomicAnd(&cbits[loc >> 5], ~(1u << (loc & 31u)));
         }
@@ -1016,10 +1052,11 @@ k_flip(const SweepArgs a)
 // ---------------------------------------------------------------------------------------------
 // Small utility kernels (init, export, debug).
 // ---------------------------------------------------------------------------------------------
-__global__ void k_init_hot(float *theta, uint64_t N, uint32_t seed_lo, uint32_t seed_hi)
+// first: index in the whole lattice of the state's first site (a slab starts at row y_off)
+__global__ void k_init_hot(float *theta, uint64_t N, uint64_t first, uint32_t seed_lo, uint32_t seed_hi)
 {
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (uint64_t)gridDim.x * blockDim.x) {
-        const U4 w = rng(seed_lo, seed_hi, i, 0u, TAG_INIT);
+        const U4 w = rng(seed_lo, seed_hi, first + i, 0u, TAG_INIT);
         const double frac = (double)(w.x >> 8) * (1.0 / 16777216.0);
         theta[i] = __double2float_rn(__dmul_rn(kTwoPi, frac));
     }

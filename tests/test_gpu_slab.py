@@ -1,0 +1,87 @@
+"""Row-slab sharded sweep on ONE GPU: G slab states of one process, driven by the same
+ShardedLattice.sweep the NCCL path uses (ranks are threads, host-side rendezvous only), against the oracle's sweep of
+the whole lattice: angles, bonds and canonical labels bit for bit, counts equal, sums to 1e-9 N."""
+import numpy as np
+import pytest
+
+from oracle import xy_oracle as xo
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def xy():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1210_6116_b200 as m
+    return m
+
+
+def _run(xy, L, G, seed, init, beta, sweeps, flags=0, check_every=1):
+    from paper_1210_6116_b200 import shard
+    kind = xy.INIT_HOT if init == "hot" else xy.INIT_COLD
+    ref = xo.init(L, seed, xo.INIT_HOT if init == "hot" else xo.INIT_COLD)
+    N = L * L
+
+    def body(rank, comm):
+        rows, y_off = shard.slab_rows(L, G, rank)
+        slab = xy.SlabState(L, rows, y_off, seed, kind, flags)
+        return shard.ShardedLattice(slab, comm)
+
+    lats = shard.run_threads(G, body)
+    got = np.concatenate([lat.slab.get_angles() for lat in lats])
+    assert (got == ref).all(), "initial state differs"
+    for t in range(sweeps):
+        shard.run_threads(G, lambda r, comm: lats[r].sweep(beta))
+        b, lab, o = xo.sweep(ref, L, seed, t, beta)
+        if t % check_every and t + 1 != sweeps:
+            continue
+        assert (np.concatenate([lat.slab.get_bonds() for lat in lats]) == b).all(), f"bonds differ at sweep {t}"
+        assert (np.concatenate([lat.slab.get_labels() for lat in lats]) == lab).all(), f"labels differ at sweep {t}"
+        assert (np.concatenate([lat.slab.get_angles() for lat in lats]) == ref).all(), f"angles differ at sweep {t}"
+        res = shard.run_threads(G, lambda r, comm: lats[r].measure())
+        for g in res:                                       # every rank holds the same global record
+            for k in ("E", "Mx", "My", "Cx", "Sx", "Cy", "Sy"):
+                assert abs(g[k] - getattr(o, k)) <= 1e-9 * N, (k, g[k], getattr(o, k))
+            assert (g["n_bonds_x"], g["n_bonds_y"], g["n_clusters"]) == (o.n_bonds_x, o.n_bonds_y, o.n_clusters)
+            assert g["sweep"] == t + 1
+    for lat in lats:
+        lat.slab.destroy()
+
+
+@pytest.mark.parametrize("L,G,init,beta", [(128, 1, "hot", 1.12), (128, 2, "hot", 1.12), (256, 4, "hot", 1.12),
+                                           (256, 2, "cold", 1.12), (256, 8, "hot", 0.7), (384, 3, "hot", 1.5),
+                                           (192, 2, "hot", 1.12), (512, 4, "cold", 1.11996)])
+def test_sharded_sweeps_equal_the_whole_lattice_oracle(xy, L, G, init, beta):
+    _run(xy, L, G, seed=40 + L + G, init=init, beta=beta, sweeps=6)
+
+
+def test_sharded_chain_large_clusters(xy):
+    """cold start at low temperature: one cluster spans every slab for many sweeps (every cut root is overridden)"""
+    _run(xy, 256, 4, seed=5, init="cold", beta=3.0, sweeps=8)
+
+
+def test_sharded_beta_zero_and_huge(xy):
+    _run(xy, 128, 2, seed=6, init="hot", beta=0.0, sweeps=2)
+    _run(xy, 128, 4, seed=6, init="cold", beta=1e9, sweeps=2)
+
+
+def test_sharded_longer_chain_L1024(xy):
+    _run(xy, 1024, 4, seed=7, init="cold", beta=1.11996, sweeps=40, check_every=10)
+
+
+def test_slab_errors(xy):
+    with pytest.raises(xy.XYError):
+        xy.SlabState(128, 48, 0, 1)                 # rows not a multiple of 32
+    with pytest.raises(xy.XYError):
+        xy.SlabState(128, 64, 96, 1)                # beyond the lattice
+    with pytest.raises(xy.XYError):
+        xy.SlabState(128, 64, 0, 1, flags=xy.FLAG_LABELS64)
+    s = xy.SlabState(128, 64, 64, 1)
+    with pytest.raises(xy.XYError):
+        s.sw_sweeps(1.0, 1)                         # a slab sweeps in two phases
+    with pytest.raises(xy.XYError):
+        import torch
+        s.slab_flip(torch.zeros(2 * s.edges.numel(), dtype=torch.uint8, device="cuda"), 2, 0)   # no label phase yet
+    s.destroy()
