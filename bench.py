@@ -285,6 +285,54 @@ def potts_leg(xy, torch, L=16384, q=3, seed=13, therm=100, K=50):
             "E_per_site": o.E / N, "bond_density": (o.n_bonds_x + o.n_bonds_y) / (2 * N), "clusters_per_site": o.n_clusters / N}
 
 
+def run_sharded(args, xy, torch, grp, rank, local_rank, world):
+    """--shard: the workload's lattice as `world` row slabs, one per GPU (strong scaling)."""
+    from paper_1210_6116_b200 import shard
+    cfg_idx, L, init, seed, beta, therm = WORKLOADS[args.workload]
+    if args.beta is not None:
+        beta = args.beta
+    N, K, W = L * L, args.steps, max(args.warmup, 3)
+    rows, y_off = shard.slab_rows(L, world, rank)
+    slab = xy.SlabState(L, rows, y_off, seed, xy_inputs.INIT_CODE[init])
+    if args.obs == "none":
+        slab.set_obs_mode(xy.OBS_NONE)
+    if world > 1:
+        comm = shard.DistComm(grp.dist, rank, world)
+    else:
+        comm = shard.ThreadComm(shard.ThreadComm.Shared(1), 0)
+    lat = shard.ShardedLattice(slab, comm)
+    lat.sweep(beta, therm + W)
+    grp.barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    launches0 = slab.get_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    grp.barrier()
+    e0.record()
+    lat.sweep(beta, K)
+    e1.record()
+    grp.barrier()
+    ms = grp.max_over_ranks(e0.elapsed_time(e1))
+    clocks = sampler.stop()
+    launches = slab.get_launch_count() - launches0
+    obs = lat.measure()
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": N * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": f"{args.workload}: ONE 2D XY lattice L={L} as {world} row slab(s) of {rows} rows, {init} start "
+                                   f"seed {seed}, beta={beta}, {therm} thermalisation sweeps untimed",
+                       "L": L, "beta": beta, "parallelism": f"row slabs x{world} (shard.py)",
+                       "exchange_bytes_per_sweep_per_rank": {"all_gather_cut_records": 17 * L, "all_gather_first_rows": 4 * L}},
+            "clocks": clocks, "gpu_launches": int(launches),
+            "observables": {"sweep": obs["sweep"], "E_per_site": obs["E"] / N, "m2": (obs["Mx"] ** 2 + obs["My"] ** 2) / N ** 2,
+                            "bond_density": (obs["n_bonds_x"] + obs["n_bonds_y"]) / (2 * N), "clusters_per_site": obs["n_clusters"] / N},
+        }
+        print(json.dumps(line), flush=True)
+    slab.destroy()
+
+
 def run_reference(args, rank, world):
     """--impl reference: the CPU oracle timed on the host cores (rank 0 only)."""
     if rank != 0:
@@ -373,6 +421,9 @@ def main():
     ap.add_argument("--obs", default="all", choices=["all", "none"],
                     help="none: time the sweeps with the observable sums switched off (xy_set_obs_mode); not the headline")
     ap.add_argument("--e2e-steps", type=int, default=None)
+    ap.add_argument("--shard", action="store_true",
+                    help="ONE lattice split into --gpus row slabs (SURVEY 8(f) #3): strong scaling, NCCL all-gather of the "
+                         "cut records and first rows every sweep; with --gpus 1 the single slab stitches onto itself")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-also", action="store_true",
@@ -395,6 +446,11 @@ def main():
     torch.cuda.set_device(local_rank)
     grp = RankGroup(rank, world, "nccl", torch.device("cuda", local_rank), torch.cuda.synchronize)
     barrier, max_over_ranks = grp.barrier, grp.max_over_ranks
+
+    if args.shard:
+        run_sharded(args, xy, torch, grp, rank, local_rank, world)
+        grp.close()
+        return
 
     cfg_idx, L, init, seed, beta, therm = WORKLOADS[args.workload]
     if args.beta is not None:
