@@ -92,6 +92,20 @@ typedef struct {
     uint64_t trace_len;             /* out: number of decisions taken (may exceed trace_cap) */
 } xy_pcc_out;
 
+/* Controller state of the PCC driver: everything xy_pcc_continue needs beyond the configuration and the sweep counter
+ * (checkpoint = xy_get_angles + xy_get_sweep + xy_pcc_get_state), and the sums of <m^2> and chi(2 pi / L) over the measured
+ * sweeps fed to the controller so far, so that a long run needs no read-back of the per-sweep series. */
+typedef struct {
+    double   beta, dbeta;           /* beta of the next sweep, current step */
+    double   acc_e, acc_s2;         /* sums of the open window */
+    uint64_t k, n_decisions;        /* measured sweeps fed, decisions taken */
+    double   stage_sum, last_sum;   /* beta_mean bookkeeping (O8) */
+    uint64_t stage_cnt, last_cnt;
+    double   sum_m2;                /* sum over the fed sweeps of (Mx^2 + My^2) / N^2 */
+    double   sum_chik;              /* sum of (|F_x|^2 + |F_y|^2) / (2 N) (states with XY_FLAG_FOURIER, else 0) */
+    uint64_t n_acc;                 /* number of sweeps in the two sums */
+} xy_pcc_state;
+
 /* ---- the five calls of the problem statement ------------------------------------------------ */
 
 /* Create a state: L x L lattice, RNG seed, initial configuration XY_INIT_*; sweep counter t = 0.
@@ -113,6 +127,13 @@ int xy_measure(xy_state *s, xy_obs *out);
  * the whole control loop on the device; blocking.  Starts at the state's current configuration and
  * sweep counter, on the state's last-used stream.  Order of operations: DESIGN.md section 3 (O8). */
 int xy_pcc_run(xy_state *s, double beta0, double dbeta0, const xy_pcc_schedule *sched, xy_pcc_out *out);
+
+/* As xy_pcc_run, but the controller goes on from its state as it stands (after an earlier xy_pcc_run / xy_pcc_continue
+ * of this state, or xy_pcc_set_state): a run of n1 + n2 sweeps equals xy_pcc_run(n1) followed by xy_pcc_continue(n2) with
+ * discard = 0, bit for bit.  out->n_decisions and the trace count the decisions of THIS call. */
+int xy_pcc_continue(xy_state *s, const xy_pcc_schedule *sched, xy_pcc_out *out);
+int xy_pcc_get_state(xy_state *s, xy_pcc_state *out);
+int xy_pcc_set_state(xy_state *s, const xy_pcc_state *in);
 
 /* Free the state (and its device memory unless it was created on a caller workspace). */
 int xy_destroy(xy_state *s);

@@ -76,6 +76,13 @@ class _PccOut(C.Structure):
                 ("trace_cap", C.c_uint64), ("trace_len", C.c_uint64)]
 
 
+class PccState(C.Structure):
+    _fields_ = [("beta", C.c_double), ("dbeta", C.c_double), ("acc_e", C.c_double), ("acc_s2", C.c_double),
+                ("k", C.c_uint64), ("n_decisions", C.c_uint64),
+                ("stage_sum", C.c_double), ("last_sum", C.c_double), ("stage_cnt", C.c_uint64), ("last_cnt", C.c_uint64),
+                ("sum_m2", C.c_double), ("sum_chik", C.c_double), ("n_acc", C.c_uint64)]
+
+
 _vp = C.c_void_p
 _SIGS = {
     "xy_create": [C.POINTER(_vp), C.c_uint32, C.c_uint64, C.c_int],
@@ -84,6 +91,9 @@ _SIGS = {
     "xy_sw_sweeps": [_vp, C.c_double, C.c_uint64, _vp],
     "xy_measure": [_vp, C.POINTER(Obs)],
     "xy_pcc_run": [_vp, C.c_double, C.c_double, C.POINTER(PccSchedule), C.POINTER(_PccOut)],
+    "xy_pcc_continue": [_vp, C.POINTER(PccSchedule), C.POINTER(_PccOut)],
+    "xy_pcc_get_state": [_vp, C.POINTER(PccState)],
+    "xy_pcc_set_state": [_vp, C.POINTER(PccState)],
     "xy_destroy": [_vp],
     "xy_get_angles": [_vp, _vp, C.c_size_t],
     "xy_get_angles_range": [_vp, _vp, C.c_uint64, C.c_size_t],
@@ -184,15 +194,30 @@ class XYState:
         _check(_lib.xy_measure(self._h, C.byref(o)))
         return o
 
+    def pcc_get_state(self):
+        st = PccState()
+        _check(_lib.xy_pcc_get_state(self._h, C.byref(st)))
+        return st
+
+    def pcc_set_state(self, st: PccState):
+        _check(_lib.xy_pcc_set_state(self._h, C.byref(st)))
+
+    def pcc_continue(self, sched: PccSchedule, trace=True):
+        return self.pcc_run(None, sched, trace)
+
     def pcc_run(self, beta0, sched: PccSchedule, trace=True):
+        """beta0 None: xy_pcc_continue (the controller goes on from its state)"""
         out = _PccOut()
-        cap = int((sched.n_sweeps - sched.discard) // max(sched.window, 1)) if trace else 0
+        cap = int((sched.n_sweeps - sched.discard) // max(sched.window, 1)) + 1 if trace else 0
         tb = np.zeros(max(cap, 1))
         ty = np.zeros(max(cap, 1))
         out.trace_beta = tb.ctypes.data_as(C.POINTER(C.c_double))
         out.trace_bY = ty.ctypes.data_as(C.POINTER(C.c_double))
         out.trace_cap = cap
-        _check(_lib.xy_pcc_run(self._h, beta0, sched.dbeta0, C.byref(sched), C.byref(out)))
+        if beta0 is None:
+            _check(_lib.xy_pcc_continue(self._h, C.byref(sched), C.byref(out)))
+        else:
+            _check(_lib.xy_pcc_run(self._h, beta0, sched.dbeta0, C.byref(sched), C.byref(out)))
         n = min(int(out.trace_len), cap)
         return {"beta_final": out.beta_final, "dbeta_final": out.dbeta_final, "beta_mean": out.beta_mean,
                 "n_decisions": int(out.n_decisions), "trace_len": int(out.trace_len),

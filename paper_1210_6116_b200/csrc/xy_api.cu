@@ -243,12 +243,18 @@ struct PccSetup {
     unsigned long long trace_cap;
 };
 
-__global__ void k_pcc_setup(DevCtl *c, PccSetup s)
+// fresh: a new run (controller reset); else the controller continues from its state (xy_pcc_continue), only the
+// schedule and the trace arrays of this call are set
+__global__ void k_pcc_setup(DevCtl *c, PccSetup s, int fresh)
 {
     if (threadIdx.x == 0 && blockIdx.x == 0) {
-        c->beta = s.beta0; c->dbeta = s.dbeta0;
-        c->acc_e = 0; c->acc_s2 = 0; c->k = 0; c->n_dec = 0;
-        c->stage_sum = 0; c->last_sum = 0; c->stage_cnt = 0; c->last_cnt = 0;
+        if (fresh) {
+            c->beta = s.beta0; c->dbeta = s.dbeta0;
+            c->acc_e = 0; c->acc_s2 = 0; c->k = 0; c->n_dec = 0;
+            c->stage_sum = 0; c->last_sum = 0; c->stage_cnt = 0; c->last_cnt = 0;
+            c->sum_m2 = 0; c->sum_chik = 0; c->n_acc = 0;
+        }
+        c->trace_base = c->n_dec;
         c->halve_every = s.halve_every; c->dbeta_min = s.dbeta_min; c->target = s.target;
         c->window = s.window; c->dirs = s.dirs;
         c->trace_beta = s.trace_beta; c->trace_bY = s.trace_bY; c->trace_cap = s.trace_cap;
@@ -677,18 +683,26 @@ int xy_measure(xy_state *s, xy_obs *out)
     return XY_OK;
 }
 
-int xy_pcc_run(xy_state *s, double beta0, double dbeta0, const xy_pcc_schedule *sc, xy_pcc_out *out)
+static int pcc_loop(xy_state *s, double beta0, double dbeta0, const xy_pcc_schedule *sc, xy_pcc_out *out, bool fresh)
 {
     if (!s || !sc || !out) return fail(XY_ERR_ARG, "NULL argument");
-    if (!(beta0 >= 0.0) || !std::isfinite(beta0) || !(dbeta0 >= 0.0) || !std::isfinite(dbeta0))
+    if (fresh && (!(beta0 >= 0.0) || !std::isfinite(beta0) || !(dbeta0 >= 0.0) || !std::isfinite(dbeta0)))
         return fail(XY_ERR_ARG, "beta0 and dbeta0 must be finite and >= 0");
     if (sc->window < 1 || (sc->dirs != 1 && sc->dirs != 2)) return fail(XY_ERR_ARG, "window must be >= 1 and dirs 1 or 2");
     if (sc->discard > sc->n_sweeps) return fail(XY_ERR_ARG, "discard > n_sweeps");
     if (s->T + sc->n_sweeps > 0xffffffffull) return fail(XY_ERR_STATE, "sweep counter would reach 2^32");
     if (s->slab) return fail(XY_ERR_STATE, "the PCC controller needs the sums of the whole lattice: not available on a slab");
     DeviceGuard g(s->device);
+    // measured sweeps the controller has been fed before this call (0 for a fresh run)
+    uint64_t k0 = 0;
+    if (!fresh) {
+        DevCtl h0;
+        CUDA_TRY(cudaMemcpyAsync(&h0, s->ctl(), sizeof h0, cudaMemcpyDeviceToHost, s->stream));
+        CUDA_TRY(cudaStreamSynchronize(s->stream));
+        k0 = h0.k;
+    }
     const uint64_t measured = sc->n_sweeps - sc->discard;
-    const uint64_t max_dec = measured / sc->window;
+    const uint64_t max_dec = (k0 + measured) / sc->window - k0 / sc->window;
     double *d_trace = nullptr;
     if (max_dec > 0) CUDA_TRY(cudaMalloc(&d_trace, max_dec * 2 * sizeof(double)));
     PccSetup ps;
@@ -696,14 +710,14 @@ int xy_pcc_run(xy_state *s, double beta0, double dbeta0, const xy_pcc_schedule *
     ps.halve_every = sc->halve_every; ps.dbeta_min = sc->dbeta_min; ps.target = sc->target;
     ps.window = sc->window; ps.dirs = sc->dirs;
     ps.trace_beta = d_trace; ps.trace_bY = d_trace ? d_trace + max_dec : nullptr; ps.trace_cap = max_dec;
-    k_pcc_setup<<<1, 32, 0, s->stream>>>(s->ctl(), ps);
+    k_pcc_setup<<<1, 32, 0, s->stream>>>(s->ctl(), ps, fresh ? 1 : 0);
     int rc = XY_OK;
-    bool feed_next = false;        // the next k_bonds_label feeds the record of the incoming state
+    bool feed_next = false;        // the next k_bonds feeds the record of the incoming state
     for (uint64_t n = 0; n < sc->n_sweeps && rc == XY_OK; ++n) {
         rc = enqueue_sweep(s, beta0, 1, feed_next ? 1 : 0);
         feed_next = false;
         if (rc != XY_OK || n < sc->discard) continue;
-        const uint64_t k = n - sc->discard + 1;
+        const uint64_t k = k0 + n - sc->discard + 1;
         const bool decision = (k % sc->window) == 0;
         if (decision || n + 1 == sc->n_sweeps) rc = ensure_obs(s, 1);   // beta must move before the next sweep reads it
         else feed_next = true;
@@ -712,11 +726,15 @@ int xy_pcc_run(xy_state *s, double beta0, double dbeta0, const xy_pcc_schedule *
     if (rc == XY_OK) {
         cudaError_t e = cudaMemcpyAsync(&h, s->ctl(), sizeof h, cudaMemcpyDeviceToHost, s->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+        const uint64_t ndec = e == cudaSuccess ? h.n_dec - h.trace_base : 0;
         if (e == cudaSuccess && d_trace && out->trace_beta && out->trace_bY && out->trace_cap) {
-            const uint64_t ncopy = h.n_dec < out->trace_cap ? h.n_dec : out->trace_cap;
+            const uint64_t ncopy = ndec < out->trace_cap ? ndec : out->trace_cap;
             e = cudaMemcpy(out->trace_beta, d_trace, ncopy * sizeof(double), cudaMemcpyDeviceToHost);
             if (e == cudaSuccess) e = cudaMemcpy(out->trace_bY, d_trace + max_dec, ncopy * sizeof(double), cudaMemcpyDeviceToHost);
         }
+        // the trace arrays of this call are about to be freed: the controller must not keep pointers to them
+        if (e == cudaSuccess) e = cudaMemsetAsync(&s->ctl()->trace_beta, 0, 2 * sizeof(double *), s->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
         if (e != cudaSuccess) rc = fail(XY_ERR_CUDA, "PCC run failed: %s", cudaGetErrorString(e));
     } else {
         cudaStreamSynchronize(s->stream);
@@ -725,11 +743,54 @@ int xy_pcc_run(xy_state *s, double beta0, double dbeta0, const xy_pcc_schedule *
     if (rc != XY_OK) return rc;
     out->beta_final = h.beta;
     out->dbeta_final = h.dbeta;
-    out->n_decisions = h.n_dec;
-    out->trace_len = h.n_dec;
+    out->n_decisions = h.n_dec - h.trace_base;
+    out->trace_len = h.n_dec - h.trace_base;
     if (h.stage_cnt > 0) out->beta_mean = h.stage_sum / (double)h.stage_cnt;
     else if (h.last_cnt > 0) out->beta_mean = h.last_sum / (double)h.last_cnt;
     else out->beta_mean = h.beta;
+    return XY_OK;
+}
+
+int xy_pcc_run(xy_state *s, double beta0, double dbeta0, const xy_pcc_schedule *sc, xy_pcc_out *out)
+{
+    return pcc_loop(s, beta0, dbeta0, sc, out, true);
+}
+
+int xy_pcc_continue(xy_state *s, const xy_pcc_schedule *sc, xy_pcc_out *out)
+{
+    return pcc_loop(s, 0.0, 0.0, sc, out, false);
+}
+
+int xy_pcc_get_state(xy_state *s, xy_pcc_state *out)
+{
+    if (!s || !out) return fail(XY_ERR_ARG, "NULL argument");
+    DeviceGuard g(s->device);
+    DevCtl h;
+    CUDA_TRY(cudaMemcpyAsync(&h, s->ctl(), sizeof h, cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    out->beta = h.beta; out->dbeta = h.dbeta; out->acc_e = h.acc_e; out->acc_s2 = h.acc_s2;
+    out->k = h.k; out->n_decisions = h.n_dec;
+    out->stage_sum = h.stage_sum; out->last_sum = h.last_sum; out->stage_cnt = h.stage_cnt; out->last_cnt = h.last_cnt;
+    out->sum_m2 = h.sum_m2; out->sum_chik = h.sum_chik; out->n_acc = h.n_acc;
+    return XY_OK;
+}
+
+int xy_pcc_set_state(xy_state *s, const xy_pcc_state *in)
+{
+    if (!s || !in) return fail(XY_ERR_ARG, "NULL argument");
+    if (!(in->beta >= 0.0) || !std::isfinite(in->beta) || !(in->dbeta >= 0.0) || !std::isfinite(in->dbeta))
+        return fail(XY_ERR_ARG, "beta and dbeta must be finite and >= 0");
+    DeviceGuard g(s->device);
+    DevCtl h;
+    CUDA_TRY(cudaMemcpyAsync(&h, s->ctl(), sizeof h, cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    h.beta = in->beta; h.dbeta = in->dbeta; h.acc_e = in->acc_e; h.acc_s2 = in->acc_s2;
+    h.k = in->k; h.n_dec = in->n_decisions;
+    h.stage_sum = in->stage_sum; h.last_sum = in->last_sum; h.stage_cnt = in->stage_cnt; h.last_cnt = in->last_cnt;
+    h.sum_m2 = in->sum_m2; h.sum_chik = in->sum_chik; h.n_acc = in->n_acc;
+    h.trace_beta = nullptr; h.trace_bY = nullptr; h.trace_cap = 0;
+    CUDA_TRY(cudaMemcpyAsync(s->ctl(), &h, sizeof h, cudaMemcpyHostToDevice, s->stream));
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
     return XY_OK;
 }
 

@@ -41,10 +41,15 @@ struct DevCtl {
     // trace
     double  *trace_beta, *trace_bY;
     unsigned long long trace_cap;
+    unsigned long long trace_base;   // decisions taken before this call: entry n_dec - trace_base of the trace arrays
     // misc
     unsigned long long fallback_count;
     unsigned int ticket;          // last-block-done counter of k_bonds
     unsigned int pad;
+    // sums over the measured sweeps fed to the controller (xy_pcc_state): <m^2> and chi(k) of a long run without
+    // reading the per-sweep ring back
+    double   sum_m2, sum_chik;
+    unsigned long long n_acc;
 };
 
 struct SweepArgs {
@@ -101,8 +106,11 @@ __device__ __forceinline__ void load_vec(const float *p, float (&out)[VEC])
 }
 
 // PCC controller step, the arithmetic of DESIGN.md section 3 (O8) in this exact order.
-__device__ inline void pcc_feed(DevCtl *c, double N, double Cx, double Sx, double Cy, double Sy)
+__device__ inline void pcc_feed(DevCtl *c, double N, double Cx, double Sx, double Cy, double Sy, double Mx, double My, double chik)
 {
+    c->sum_m2 = __dadd_rn(c->sum_m2, __ddiv_rn(__dadd_rn(__dmul_rn(Mx, Mx), __dmul_rn(My, My)), __dmul_rn(N, N)));
+    c->sum_chik = __dadd_rn(c->sum_chik, chik);
+    c->n_acc += 1;
     double e, s2;
     if (c->dirs == 2) {
         e = __ddiv_rn(__dadd_rn(Cx, Cy), __dmul_rn(2.0, N));
@@ -123,9 +131,9 @@ __device__ inline void pcc_feed(DevCtl *c, double N, double Cx, double Sx, doubl
         const double bn = __dmul_rn(c->beta, N);
         const double Y = __dsub_rn(ae, __dmul_rn(bn, as2));
         const double bY = __dmul_rn(c->beta, Y);
-        if (c->trace_beta && c->n_dec < c->trace_cap) {
-            c->trace_beta[c->n_dec] = c->beta;
-            c->trace_bY[c->n_dec] = bY;
+        if (c->trace_beta && c->n_dec - c->trace_base < c->trace_cap) {
+            c->trace_beta[c->n_dec - c->trace_base] = c->beta;
+            c->trace_bY[c->n_dec - c->trace_base] = bY;
         }
         c->stage_sum = __dadd_rn(c->stage_sum, c->beta);
         c->stage_cnt += 1;
@@ -562,7 +570,14 @@ k_bonds(const SweepArgs a)
                     o->Mx = tot[0]; o->My = tot[1]; o->Cx = tot[2]; o->Sx = tot[3]; o->Cy = tot[4]; o->Sy = tot[5];
                     o->E = -(tot[2] + tot[4]);
                 }
-                if (a.feed_pcc) pcc_feed(a.ctl, N, tot[2], tot[3], tot[4], tot[5]);
+                if (a.feed_pcc) {
+                    double chik = 0.0;                                  // (|F_x|^2 + |F_y|^2) / (2 N), Eq. 9 at k = 2 pi / L
+                    if constexpr (kFourier) {
+                        for (int k = 6; k < 14; ++k) chik = __fma_rn(tot[k], tot[k], chik);
+                        chik = __ddiv_rn(chik, __dmul_rn(2.0, N));
+                    }
+                    pcc_feed(a.ctl, N, tot[2], tot[3], tot[4], tot[5], tot[0], tot[1], chik);
+                }
             }
             if constexpr (kBonds) {
                 xy_obs *o = a.ring + ((a.t + 1u) % a.ring_cap);  // record of T = t+1, completed later

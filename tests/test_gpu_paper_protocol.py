@@ -2,8 +2,9 @@
 1000 MCS, dbeta = 5e-4, 60 000 MCS discarded), shortened to 3e5 measured sweeps, against Table I
 (PAPER.md:80-88): beta_KT(L), <m^2>_L and xi_2nd(L)/L for L = 64 ... 1024 by default (L = 2048 and 4096 with
 XY_LONG=1: 40 s and 80 s of GPU time).  Statistical pins with the error bar of THIS run: the beta trace is
-binned into 10 blocks of 30 windows, the last 16 000 sweeps of the series into 16 blocks of 1000 sweeps
-(xi_2nd by jackknife over the blocks); a value passes if it is within 5 combined standard errors (ours and the
+binned into 10 blocks of 30 windows; <m^2> and chi(2 pi / L) come from the controller's device-side sums over ALL 3e5
+measured sweeps, read after each of ten chunks (xy_pcc_run + 9 x xy_pcc_continue), xi_2nd by jackknife over the ten
+blocks; a value passes if it is within 5 combined standard errors (ours and the
 paper's, which are for 4e6 MCS) AND within a fixed cap that keeps the check meaningful should the binned
 error come out large."""
 import os
@@ -43,28 +44,34 @@ def test_paper_protocol_table1(xy, L, seed):
     c = constants()
     target, dbeta = c["betaY_critical"], c["pcc_dbeta"]
     assert (int(c["pcc_window_mcs"]), int(c["pcc_discard_mcs"])) == (1000, 60000)
-    discard, windows = 60000, 300
-    sched = xy.PccSchedule(n_sweeps=discard + 1000 * windows, discard=discard, window=1000, dirs=1,
-                           dbeta0=dbeta, halve_every=0, dbeta_min=dbeta, target=target)
+    discard, windows, nb = 60000, 300, 10
+    mk = lambda n, disc: xy.PccSchedule(n_sweeps=n, discard=disc, window=1000, dirs=1, dbeta0=dbeta, halve_every=0,
+                                        dbeta_min=dbeta, target=target)
     st = xy.XYState(L, seed, xy.INIT_HOT, flags=xy.FLAG_FOURIER)
-    out = st.pcc_run(1.10, sched)
-    tb = out["trace_beta"]
-    assert out["n_decisions"] == windows and tb.size == windows
+    # ten chunks of 30 windows: xy_pcc_run, then xy_pcc_continue; the controller's own sums of <m^2> and chi(k) over ALL
+    # measured sweeps are read after every chunk (xy_pcc_get_state), which gives ten block means without reading
+    # 3e5 records back
+    per = 1000 * windows // nb
+    tb, m2s, fks = [], [], []
+    prev = None
+    for b in range(nb):
+        out = st.pcc_run(1.10, mk(discard + per, discard)) if b == 0 else st.pcc_continue(mk(per, 0))
+        assert out["n_decisions"] == windows // nb
+        tb.append(out["trace_beta"])
+        cs = st.pcc_get_state()
+        base = (0.0, 0.0, 0) if prev is None else prev
+        assert cs.n_acc - base[2] == per
+        m2s.append((cs.sum_m2 - base[0]) / per)
+        fks.append((cs.sum_chik - base[1]) / per)
+        prev = (cs.sum_m2, cs.sum_chik, cs.n_acc)
+    tb, m2s, fks = np.concatenate(tb), np.array(m2s), np.array(fks)
+    assert tb.size == windows
     beta_kt = tb.mean()
-    # beta walks in steps of 5e-4 around the crossing: error of the mean from 10 blocks of 30 windows
-    bb = tb.reshape(10, 30).mean(axis=1)
-    beta_err = bb.std(ddof=1) / np.sqrt(bb.size)
+    # beta walks in steps of 5e-4 around the crossing: error of the mean from the 10 blocks of 30 windows
+    bb = tb.reshape(nb, -1).mean(axis=1)
+    beta_err = bb.std(ddof=1) / np.sqrt(nb)
     _within("beta_KT", beta_kt, beta_err, row["beta"], row["beta_err"], 2.5e-3)
-    # <m^2> and xi_2nd / L over the records the device ring still holds (the last 16383 sweeps of the walk)
-    T = st.get_sweep()
-    cap = st.series_capacity()
-    n = min(cap - 1, 16000)
-    obs = st.get_series(T - n + 1, n)
-    fou = st.get_fourier_series(T - n + 1, n)
     N = L * L
-    nb = 16
-    m2s = ((obs["Mx"] ** 2 + obs["My"] ** 2) / N ** 2).reshape(nb, -1).mean(axis=1)
-    fks = (0.5 * ((fou["Fx"] ** 2).sum(axis=1) + (fou["Fy"] ** 2).sum(axis=1)) / N).reshape(nb, -1).mean(axis=1)
     m2 = m2s.mean()
     m2_err = m2s.std(ddof=1) / np.sqrt(nb)
     _within("<m^2>", m2, m2_err, row["m2"], row["m2_err"], 0.005)
@@ -72,6 +79,22 @@ def test_paper_protocol_table1(xy, L, seed):
     jk = np.array([xo.xi2nd(N * np.delete(m2s, b).mean(), np.delete(fks, b).mean(), L) / L for b in range(nb)])
     xi_err = np.sqrt((nb - 1) / nb * ((jk - jk.mean()) ** 2).sum())
     _within("xi_2nd/L", xi_over_L, xi_err, row["xi"], row["xi_err"], 0.012)
+    # the device-side sums agree with the records the ring still holds (the last sweeps of the walk)
+    T = st.get_sweep()
+    n = 4000
+    obs = st.get_series(T - n + 1, n)
+    fou = st.get_fourier_series(T - n + 1, n)
+    tail_m2 = ((obs["Mx"] ** 2 + obs["My"] ** 2) / float(N) ** 2)
+    tail_fk = 0.5 * ((fou["Fx"] ** 2).sum(axis=1) + (fou["Fy"] ** 2).sum(axis=1)) / N
+    st2 = xy.XYState(L, seed, xy.INIT_HOT, flags=xy.FLAG_FOURIER)   # a second, short run pins the sums sweep by sweep
+    st2.pcc_run(1.10, mk(300, 100))
+    c2 = st2.pcc_get_state()
+    o2, f2 = st2.get_series(101, 200), st2.get_fourier_series(101, 200)
+    want_m2 = ((o2["Mx"] ** 2 + o2["My"] ** 2) / float(N) ** 2).sum()
+    want_fk = (0.5 * ((f2["Fx"] ** 2).sum(axis=1) + (f2["Fy"] ** 2).sum(axis=1)) / N).sum()
+    assert c2.n_acc == 200 and abs(c2.sum_m2 - want_m2) <= 1e-12 * want_m2 and abs(c2.sum_chik - want_fk) <= 1e-12 * want_fk
+    assert abs(tail_m2.mean() - m2) < 0.05 * m2 and abs(tail_fk.mean() - fks.mean()) < 0.1 * fks.mean()
+    st2.destroy()
     print(f"L={L}: beta_KT {beta_kt:.5f}({beta_err:.5f}) (paper {row['beta']}({row['beta_err']})), "
           f"m2 {m2:.5f}({m2_err:.5f}) (paper {row['m2']}({row['m2_err']})), "
           f"xi/L {xi_over_L:.4f}({xi_err:.4f}) (paper {row['xi']}({row['xi_err']}))")

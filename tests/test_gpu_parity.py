@@ -341,3 +341,38 @@ def test_errors(xy):
     st.sw_sweeps(1.0, 2)
     assert st.measure().sweep == 2
     st.destroy()
+
+
+def test_pcc_continue_and_checkpoint(xy):
+    """xy_pcc_run(2 M) == xy_pcc_run(M) + xy_pcc_continue(M), also through a checkpoint into a fresh state (angles, sweep
+    counter, controller state); the device-side sums of <m^2> equal the per-sweep series of the fed sweeps."""
+    L, seed, M = 128, 9, 240
+    mk = lambda n, disc: xy.PccSchedule(n_sweeps=n, discard=disc, window=20, dirs=1, dbeta0=1e-3, halve_every=100,
+                                        dbeta_min=1e-6, target=2 / np.pi)
+    a = xy.XYState(L, seed, xy.INIT_HOT)
+    ra = a.pcc_run(1.05, mk(2 * M + 10, 10))
+    b = xy.XYState(L, seed, xy.INIT_HOT)
+    r1 = b.pcc_run(1.05, mk(M + 10, 10))
+    r2 = b.pcc_continue(mk(M, 0))
+    assert r2["beta_final"] == ra["beta_final"] and r2["dbeta_final"] == ra["dbeta_final"]
+    assert (np.concatenate([r1["trace_beta"], r2["trace_beta"]]) == ra["trace_beta"]).all()
+    assert (np.concatenate([r1["trace_bY"], r2["trace_bY"]]) == ra["trace_bY"]).all()
+    assert (a.get_angles() == b.get_angles()).all()
+    # checkpoint after the first part, restore into another state
+    c = xy.XYState(L, seed, xy.INIT_HOT)
+    c.pcc_run(1.05, mk(M + 10, 10))
+    ck = (c.get_angles(), c.get_sweep(), c.pcc_get_state())
+    d = xy.XYState(L, seed, xy.INIT_COLD)                 # the seed belongs to the checkpoint: same RNG stream
+    d.set_angles(ck[0]); d.set_sweep(ck[1]); d.pcc_set_state(ck[2])
+    r3 = d.pcc_continue(mk(M, 0))
+    assert r3["beta_final"] == ra["beta_final"] and (r3["trace_beta"] == r2["trace_beta"]).all()
+    assert (d.get_angles() == a.get_angles()).all()
+    sa, sd = a.pcc_get_state(), d.pcc_get_state()
+    assert (sa.k, sa.n_decisions, sa.n_acc) == (sd.k, sd.n_decisions, sd.n_acc) == (2 * M, 2 * M // 20, 2 * M)
+    assert sa.sum_m2 == sd.sum_m2 and sa.beta == sd.beta
+    # the fed sweeps are the states T = 11 ... 2 M + 10 of run a
+    ser = a.get_series(11, 2 * M)
+    m2 = ((ser["Mx"] ** 2 + ser["My"] ** 2) / float(L * L) ** 2).sum()
+    assert abs(sa.sum_m2 - m2) <= 1e-12 * m2
+    for s in (a, b, c, d):
+        s.destroy()
