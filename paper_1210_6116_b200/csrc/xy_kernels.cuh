@@ -998,9 +998,11 @@ k_flip(const SweepArgs a)
                 while (!((uint32_t)root & kSlabSpecial)) {
                     const LabelT p = __ldg(labels + root);
                     if (p == root) break;
+                    XY_CHECK(CHK_GLABEL, ((uint32_t)p & kSlabSpecial) || p < root);
                     root = p;
                 }
                 if ((uint32_t)root & kSlabSpecial) {
+                    XY_CHECK(CHK_GLABEL, ((uint32_t)root & ~kSlabSpecial) < 2u * L);
                     groot = a.xroot[(uint32_t)root & ~kSlabSpecial];
                     if (groot == (uint64_t)self + goff) ++ncl;   // the cluster's canonical root is this very site
                 } else {

@@ -6,7 +6,8 @@
 
 Two sweeps plus the getters at L = 64 and L = 1024 for both label widths, with the structure-factor sums
 on and off and with the observables switched off: every kernel variant these sizes select runs at least
-once.  Results are summarised in profiles/r2_sanitizers.md."""
+once.  The Potts sweep and the row-slab path follow.  Results are summarised in
+profiles/r2_checked_build.md."""
 import os
 import sys
 
@@ -36,6 +37,26 @@ def main():
             st.sw_sweeps(1.11996, n)
             print(L, flags, st.measure().n_clusters, st.debug_check_labels())
             st.destroy()
+    # the Potts sweep and the row-slab path (two slabs of one process) on the same labeling kernels
+    for L, q in ((64, 2), (192, 3), (1024, 5)):
+        ps = xy.PottsState(L, q, 3, xy.INIT_HOT)
+        ps.sweeps(1.0, 3)
+        o = ps.measure()
+        ps.get_bonds(); ps.get_labels(); ps.get_spins()
+        print("potts", L, q, o.n_clusters, o.E)
+        ps.destroy()
+    from paper_1210_6116_b200 import shard
+    for L, G in ((128, 2), (192, 2), (1024, 4)):
+        def body(rank, comm):
+            rows, y_off = shard.slab_rows(L, G, rank)
+            return shard.ShardedLattice(xy.SlabState(L, rows, y_off, 3, xy.INIT_HOT), comm)
+        lats = shard.run_threads(G, body)
+        shard.run_threads(G, lambda r, comm: lats[r].sweep(1.12, 3))
+        res = shard.run_threads(G, lambda r, comm: lats[r].measure())
+        for lat in lats:
+            lat.slab.get_labels(); lat.slab.get_bonds()
+            lat.slab.destroy()
+        print("slabs", L, G, res[0]["n_clusters"])
     counts, checked = xy.debug_check_counts()
     print("checked build:", checked, "range-check violations:", counts)
     assert sum(counts) == 0
