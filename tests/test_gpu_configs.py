@@ -143,9 +143,10 @@ def test_config3_first_40_sweeps_chained(xy):
 
 
 def test_config3_pcc_trace_L256(xy):
-    """config 3's schedule, shortened in proportion (8000 sweeps, dbeta halved every 800), chained at L = 256"""
-    n = 8000
-    cfg, sg, so = _cfg3_schedules(xy, n, halve=800)
+    """config 3's schedule, shortened in proportion (4000 sweeps = 200 decisions, dbeta halved every 400), chained
+    at L = 256 (the oracle's share of this test is 50 s)"""
+    n = 4000
+    cfg, sg, so = _cfg3_schedules(xy, n, halve=400)
     L, seed = 256, cfg["seed"]
     st = xy.XYState(L, seed, xy.INIT_HOT)
     out = st.pcc_run(cfg["beta0"], sg)
