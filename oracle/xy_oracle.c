@@ -48,6 +48,10 @@
  *   fourier     : numpy FFT of the spin field; plane wave and uniform closed forms;
  *                 Eq. 8 inverts the Ornstein-Zernike form exactly; xi_2nd/L of the
  *                 paper's Table I row L=64.
+ *   potts       : (section at the end of this file; tests/test_oracle_potts.py) exact one-step transition
+ *                 matrix and Boltzmann weights of the 2x2 torus (q = 3), enumeration of all 2^16 states
+ *                 of the 4x4 q = 2 model, bond-rule closed forms, uniformity and independence of the
+ *                 fresh spins, e(beta_c) = -(1 + 1/sqrt q) at the self-dual point.
  * No function here is "parity unpinned".
  */
 #include <math.h>
