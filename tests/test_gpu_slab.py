@@ -18,7 +18,7 @@ def xy():
     return m
 
 
-def _run(xy, L, G, seed, init, beta, sweeps, flags=0, check_every=1):
+def _run(xy, L, G, seed, init, beta, sweeps, flags=0, check_every=1, obs_none=False):
     from paper_1210_6116_b200 import shard
     kind = xy.INIT_HOT if init == "hot" else xy.INIT_COLD
     ref = xo.init(L, seed, xo.INIT_HOT if init == "hot" else xo.INIT_COLD)
@@ -27,6 +27,8 @@ def _run(xy, L, G, seed, init, beta, sweeps, flags=0, check_every=1):
     def body(rank, comm):
         rows, y_off = shard.slab_rows(L, G, rank)
         slab = xy.SlabState(L, rows, y_off, seed, kind, flags)
+        if obs_none:
+            slab.set_obs_mode(xy.OBS_NONE)           # chained sweeps without the sums; measure still works
         return shard.ShardedLattice(slab, comm)
 
     lats = shard.run_threads(G, body)
@@ -69,6 +71,12 @@ def test_sharded_beta_zero_and_huge(xy):
 
 def test_sharded_longer_chain_L1024(xy):
     _run(xy, 1024, 4, seed=7, init="cold", beta=1.11996, sweeps=40, check_every=10)
+
+
+def test_sharded_without_observables(xy):
+    """the k_bonds variant without the fp64 sums (xy_set_obs_mode) on slabs, both tile widths"""
+    _run(xy, 256, 2, seed=8, init="hot", beta=1.12, sweeps=5, obs_none=True, check_every=2)
+    _run(xy, 192, 2, seed=8, init="hot", beta=1.12, sweeps=3, obs_none=True)
 
 
 def test_slab_errors(xy):
