@@ -35,8 +35,10 @@ struct PottsArgs {
 
 __device__ __forceinline__ uint32_t eq4_bits(uint32_t a, uint32_t b)   // bit j = byte j of a equals byte j of b
 {
-    const uint32_t m = __vcmpeq4(a, b) & 0x01010101u;
-    return (m | (m >> 7) | (m >> 14) | (m >> 21)) & 15u;
+    // spins are below 128: the low 7 bits of a byte of a ^ b are zero iff the bytes are equal, and adding 0x7f then
+    // leaves bit 7 clear exactly there (no carry crosses a byte)
+    const uint32_t m = ~((a ^ b) + 0x7f7f7f7fu) & 0x80808080u;
+    return (m >> 7 | m >> 14 | m >> 21 | m >> 28) & 15u;
 }
 
 // kBonds = false: observables only (xy_potts_measure of a state no sweep has looked at yet).  KQ: number of spin
@@ -65,27 +67,36 @@ k_potts_bonds(const PottsArgs a)
         const uint32_t eqy = eq4_bits(own, down);
         ex += __popc(eqx);
         ey += __popc(eqy);
+        if constexpr (KQ == 4) {                     // two bits per spin: four masks from two bit planes
+            const uint32_t b0 = own & 0x01010101u, b1 = (own >> 1) & 0x01010101u;
+            cnt[3] += __popc(b0 & b1);
+            cnt[1] += __popc(b0 & ~b1);
+            cnt[2] += __popc(b1 & ~b0);
+            cnt[0] += __popc(0x01010101u & ~(b0 | b1));
+        } else {
 #pragma unroll
-        for (int k = 0; k < KQ; ++k) cnt[k] += __popc(__vcmpeq4(own, 0x01010101u * (uint32_t)k) & 0x01010101u);
+            for (int k = 0; k < KQ; ++k) cnt[k] += __popc(eq4_bits(own, 0x01010101u * (uint32_t)k));
+        }
         if constexpr (kBonds) {
             const U4 wA = rng(a.seed_lo, a.seed_hi, qd, a.t, TAG_BOND);
             const uint32_t w[4] = {wA.x, wA.y, wA.z, wA.w};
-            uint32_t xn = 0, yn = 0, open = 0;
+            // h < Th as the sign of h - Th (both below 2^17), shifted into place by funnel shifts
+            uint32_t xn = 0, yn = 0;
+            bool tie = false;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const uint32_t hx = w[j] & 0xffffu, hy = w[j] >> 16;
-                xn |= (hx < Th ? 1u : 0u) << j;
-                yn |= (hy < Th ? 1u : 0u) << j;
-                open |= (hx == Th ? 1u : 0u) << j;
-                open |= (hy == Th ? 16u : 0u) << j;
+            for (int j = 3; j >= 0; --j) {
+                const uint32_t dx = (w[j] & 0xffffu) - Th, dy = (w[j] >> 16) - Th;
+                xn = __funnelshift_l(dx, xn, 1);
+                yn = __funnelshift_l(dy, yn, 1);
+                tie = tie || dx == 0u || dy == 0u;
             }
-            if (open & (eqx | (eqy << 4))) {               // rare (2^-16 per decision): the trailing 16 bits decide
+            if (tie) {                                     // rare (2^-16 per decision): the trailing 16 bits decide
                 const U4 wB = rng(a.seed_lo, a.seed_hi, qd, a.t, TAG_BOND_LO);
                 const uint32_t v[4] = {wB.x, wB.y, wB.z, wB.w};
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
-                    if ((open >> j) & 1u) xn |= ((v[j] & 0xffffu) < Tl ? 1u : 0u) << j;
-                    if ((open >> (4 + j)) & 1u) yn |= ((v[j] >> 16) < Tl ? 1u : 0u) << j;
+                    if ((w[j] & 0xffffu) == Th) xn |= ((v[j] & 0xffffu) < Tl ? 1u : 0u) << j;
+                    if ((w[j] >> 16) == Th) yn |= ((v[j] >> 16) < Tl ? 1u : 0u) << j;
                 }
             }
             xn &= eqx;
