@@ -247,6 +247,16 @@ int xy_slab_buffers(xy_state *s, void **dev_first_row, void **dev_halo_row, size
 int xy_slab_label(xy_state *s, double beta, void *cuda_stream);
 /* dev_gathered_edges: nranks edge records in rank order (device memory) */
 int xy_slab_flip(xy_state *s, const void *dev_gathered_edges, uint32_t nranks, uint32_t rank, void *cuda_stream);
+/* The PCC driver on a sharded lattice (the paper's own use of its multi-GPU code, PAPER.md:62-66 at L >= 8192): the
+ * controller (O8) runs replicated on every rank's device, fed with all-reduced sums.  Per measured sweep, after the halo
+ * exchange: xy_slab_obs_partial (the slab's six sums of the new configuration -> dev_partial8), all-reduce (sum) of the 8
+ * doubles into dev_global8 (caller), xy_slab_pcc_feed.  xy_slab_label_pcc sweeps at the controller's beta.  The
+ * controller state is read with xy_pcc_get_state; all ranks hold the same one. */
+int xy_slab_pcc_setup(xy_state *s, double beta0, double dbeta0, const xy_pcc_schedule *sched);
+int xy_slab_label_pcc(xy_state *s, void *cuda_stream);
+int xy_slab_pcc_buffers(xy_state *s, void **dev_partial8, void **dev_global8);
+int xy_slab_obs_partial(xy_state *s, void *cuda_stream);
+int xy_slab_pcc_feed(xy_state *s, void *cuda_stream);
 
 /* ---- q-state Potts model on the same labeling core ------------------------
  * PAPER.md:30-34 cites the authors' GPU Swendsen-Wang codes for the Potts and Ising models (refs 19, 22)

@@ -122,6 +122,11 @@ _SIGS = {
     "xy_slab_buffers": [_vp, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(C.c_size_t), C.POINTER(_vp), C.POINTER(C.c_size_t)],
     "xy_slab_label": [_vp, C.c_double, _vp],
     "xy_slab_flip": [_vp, _vp, C.c_uint32, C.c_uint32, _vp],
+    "xy_slab_pcc_setup": [_vp, C.c_double, C.c_double, C.POINTER(PccSchedule)],
+    "xy_slab_label_pcc": [_vp, _vp],
+    "xy_slab_pcc_buffers": [_vp, C.POINTER(_vp), C.POINTER(_vp)],
+    "xy_slab_obs_partial": [_vp, _vp],
+    "xy_slab_pcc_feed": [_vp, _vp],
     "xy_potts_create": [C.POINTER(_vp), C.c_uint32, C.c_uint32, C.c_uint64, C.c_int],
     "xy_potts_destroy": [_vp],
     "xy_potts_sweeps": [_vp, C.c_double, C.c_uint64, _vp],
@@ -376,11 +381,31 @@ class SlabState(XYState):
         self.first_row = self._ws[first.value - base: first.value - base + rb.value].view(torch.float32)
         self.halo_row = self._ws[halo.value - base: halo.value - base + rb.value].view(torch.float32)
         self.edges = self._ws[edges.value - base: edges.value - base + eb.value]
+        part, glob = _vp(), _vp()
+        _check(_lib.xy_slab_pcc_buffers(self._h, C.byref(part), C.byref(glob)))
+        self.pcc_partial = self._ws[part.value - base: part.value - base + 64].view(torch.float64)
+        self.pcc_global = self._ws[glob.value - base: glob.value - base + 64].view(torch.float64)
 
     def slab_label(self, beta, stream=None):
         import torch
         st = torch.cuda.current_stream().cuda_stream if stream is None else stream
         _check(_lib.xy_slab_label(self._h, beta, st))
+
+    def _stream(self, stream):
+        import torch
+        return torch.cuda.current_stream().cuda_stream if stream is None else stream
+
+    def slab_pcc_setup(self, beta0, sched: PccSchedule):
+        _check(_lib.xy_slab_pcc_setup(self._h, beta0, sched.dbeta0, C.byref(sched)))
+
+    def slab_label_pcc(self, stream=None):
+        _check(_lib.xy_slab_label_pcc(self._h, self._stream(stream)))
+
+    def slab_obs_partial(self, stream=None):
+        _check(_lib.xy_slab_obs_partial(self._h, self._stream(stream)))
+
+    def slab_pcc_feed(self, stream=None):
+        _check(_lib.xy_slab_pcc_feed(self._h, self._stream(stream)))
 
     def slab_flip(self, gathered, nranks, rank, stream=None):
         import torch

@@ -136,4 +136,19 @@ __global__ void k_slab_labels_to_i64(const uint32_t *labels, const uint64_t *xro
     }
 }
 
+// PCC on a sharded lattice: the slab's partial sums of one record as 8 doubles (Mx, My, Cx, Sx, Cy, Sy, 0, 0) for the
+// all-reduce, and the controller step on the all-reduced sums (replicated on every rank: same inputs, same arithmetic)
+__global__ void k_slab_pack_obs(const xy_obs *rec, double *out8)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        out8[0] = rec->Mx; out8[1] = rec->My; out8[2] = rec->Cx; out8[3] = rec->Sx; out8[4] = rec->Cy; out8[5] = rec->Sy;
+        out8[6] = 0.0; out8[7] = 0.0;
+    }
+}
+
+__global__ void k_slab_pcc_feed(DevCtl *c, const double *g8, double N)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) pcc_feed(c, N, g8[2], g8[3], g8[4], g8[5], g8[0], g8[1], 0.0);
+}
+
 }  // namespace xy

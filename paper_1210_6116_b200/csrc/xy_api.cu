@@ -46,7 +46,7 @@ constexpr size_t kStageBytes = 64u << 20;  // staging buffer of the debug getter
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-    size_t theta, labels, bonds, rootmask, partials, ring, fring, ctl, tab, edges, xroot, total;
+    size_t theta, labels, bonds, rootmask, partials, ring, fring, ctl, tab, edges, xroot, pccbuf, total;
 };
 
 // rows == L and slab == false: a whole lattice.  A slab holds `rows` rows plus one halo row of
@@ -69,6 +69,7 @@ Layout make_layout(uint32_t L, uint32_t flags, uint32_t rows = 0, bool slab = fa
     o.tab = off;      off = align_up(off + (size_t)(kTabN + 1) * sizeof(double2), 256);
     o.edges = off;    off = align_up(off + (slab ? slab_edge_bytes(L) : 0), 256);
     o.xroot = off;    off = align_up(off + (slab ? (size_t)2 * L * 8 : 0), 256);
+    o.pccbuf = off;   off = align_up(off + (slab ? (size_t)16 * 8 : 0), 256);
     o.total = off;
     return o;
 }
@@ -307,6 +308,7 @@ struct xy_state {
     double2 *tab() const { return reinterpret_cast<double2 *>(ws + lay.tab); }
     unsigned char *edges() const { return reinterpret_cast<unsigned char *>(ws + lay.edges); }
     uint64_t *xroot() const { return reinterpret_cast<uint64_t *>(ws + lay.xroot); }
+    double *pccbuf() const { return reinterpret_cast<double *>(ws + lay.pccbuf); }   // [0..7] partial, [8..15] all-reduced
     bool l64() const { return (flags & XY_FLAG_LABELS64) != 0; }
     bool fourier() const { return (flags & XY_FLAG_FOURIER) != 0; }
     xy_fourier *fring() const { return reinterpret_cast<xy_fourier *>(ws + lay.fring); }
@@ -1147,12 +1149,12 @@ int xy_slab_buffers(xy_state *s, void **dev_first_row, void **dev_halo_row, size
     return XY_OK;
 }
 
-int xy_slab_label(xy_state *s, double beta, void *cuda_stream)
+static int slab_label_common(xy_state *s, double beta, int beta_from_ctl, void *cuda_stream)
 {
     if (!s) return fail(XY_ERR_ARG, "state is NULL");
     if (!s->slab) return fail(XY_ERR_STATE, "not a slab");
     if (s->slab_labelled) return fail(XY_ERR_STATE, "xy_slab_flip of the previous xy_slab_label is pending");
-    if (!(beta >= 0.0) || !std::isfinite(beta)) return fail(XY_ERR_ARG, "beta must be finite and >= 0");
+    if (!beta_from_ctl && (!(beta >= 0.0) || !std::isfinite(beta))) return fail(XY_ERR_ARG, "beta must be finite and >= 0");
     if (s->T >= 0xffffffffull) return fail(XY_ERR_STATE, "sweep counter would reach 2^32");
     DeviceGuard g(s->device);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -1163,6 +1165,7 @@ int xy_slab_label(xy_state *s, double beta, void *cuda_stream)
     SweepArgs a = base_args(s);
     set_direction(s, s->T, a);
     a.beta = beta;
+    a.beta_from_ctl = beta_from_ctl;
     const bool with_obs = s->obs_mode == XY_OBS_ALL && s->obs_valid_T != s->T;
     a.obs_fill = with_obs ? 1 : 0;
     if (with_obs) CUDA_TRY(s->ker.bonds(a, 0, s->fourier(), s->grid_bonds, s->stream));
@@ -1176,6 +1179,64 @@ int xy_slab_label(xy_state *s, double beta, void *cuda_stream)
     if (a.obs_fill) s->obs_valid_T = s->T;
     s->pending = a;
     s->slab_labelled = true;
+    return XY_OK;
+}
+
+int xy_slab_label(xy_state *s, double beta, void *cuda_stream) { return slab_label_common(s, beta, 0, cuda_stream); }
+
+/* ---- PCC on a sharded lattice: the controller runs replicated on every rank, fed with all-reduced sums ---- */
+int xy_slab_pcc_setup(xy_state *s, double beta0, double dbeta0, const xy_pcc_schedule *sc)
+{
+    if (!s || !sc) return fail(XY_ERR_ARG, "NULL argument");
+    if (!s->slab) return fail(XY_ERR_STATE, "not a slab");
+    if (!(beta0 >= 0.0) || !std::isfinite(beta0) || !(dbeta0 >= 0.0) || !std::isfinite(dbeta0))
+        return fail(XY_ERR_ARG, "beta0 and dbeta0 must be finite and >= 0");
+    if (sc->window < 1 || (sc->dirs != 1 && sc->dirs != 2)) return fail(XY_ERR_ARG, "window must be >= 1 and dirs 1 or 2");
+    DeviceGuard g(s->device);
+    PccSetup ps;
+    ps.beta0 = beta0; ps.dbeta0 = dbeta0;
+    ps.halve_every = sc->halve_every; ps.dbeta_min = sc->dbeta_min; ps.target = sc->target;
+    ps.window = sc->window; ps.dirs = sc->dirs;
+    ps.trace_beta = nullptr; ps.trace_bY = nullptr; ps.trace_cap = 0;
+    k_pcc_setup<<<1, 32, 0, s->stream>>>(s->ctl(), ps, 1);
+    CUDA_TRY(cudaGetLastError());
+    return XY_OK;
+}
+
+int xy_slab_label_pcc(xy_state *s, void *cuda_stream) { return slab_label_common(s, 0.0, 1, cuda_stream); }
+
+int xy_slab_pcc_buffers(xy_state *s, void **dev_partial8, void **dev_global8)
+{
+    if (!s || !dev_partial8 || !dev_global8) return fail(XY_ERR_ARG, "NULL argument");
+    if (!s->slab) return fail(XY_ERR_STATE, "not a slab");
+    *dev_partial8 = s->pccbuf();
+    *dev_global8 = s->pccbuf() + 8;
+    return XY_OK;
+}
+
+int xy_slab_obs_partial(xy_state *s, void *cuda_stream)
+{
+    if (!s) return fail(XY_ERR_ARG, "state is NULL");
+    if (!s->slab) return fail(XY_ERR_STATE, "not a slab");
+    if (s->slab_labelled) return fail(XY_ERR_STATE, "xy_slab_flip is pending");
+    DeviceGuard g(s->device);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (st != s->stream) { CUDA_TRY(cudaStreamSynchronize(s->stream)); s->stream = st; }
+    if (int rc = ensure_obs(s, 0)) return rc;
+    k_slab_pack_obs<<<1, 32, 0, s->stream>>>(s->ring() + (s->T % kRingCap), s->pccbuf());
+    CUDA_TRY(cudaGetLastError());
+    return XY_OK;
+}
+
+int xy_slab_pcc_feed(xy_state *s, void *cuda_stream)
+{
+    if (!s) return fail(XY_ERR_ARG, "state is NULL");
+    if (!s->slab) return fail(XY_ERR_STATE, "not a slab");
+    DeviceGuard g(s->device);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (st != s->stream) { CUDA_TRY(cudaStreamSynchronize(s->stream)); s->stream = st; }
+    k_slab_pcc_feed<<<1, 32, 0, s->stream>>>(s->ctl(), s->pccbuf() + 8, (double)s->L * (double)s->L);
+    CUDA_TRY(cudaGetLastError());
     return XY_OK;
 }
 

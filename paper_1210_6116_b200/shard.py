@@ -83,6 +83,25 @@ class ShardedLattice:
             self.slab.slab_flip(gathered.reshape(-1), self.world, self.rank)
             self.exchange_halo()
 
+    def pcc_run(self, beta0, sched, on_decision=None):
+        """The PCC driver (O8) on the sharded lattice: the controller runs replicated on every rank's device, fed after
+        every measured sweep with the all-reduced sums of the new configuration (one 8-double all-reduce per sweep).
+        Returns the controller state (binding.PccState) of this rank; all ranks hold the same one."""
+        slab = self.slab
+        slab.slab_pcc_setup(beta0, sched)
+        for n in range(int(sched.n_sweeps)):
+            slab.slab_label_pcc()
+            gathered = self.comm.all_gather(slab.edges)
+            slab.slab_flip(gathered.reshape(-1), self.world, self.rank)
+            self.exchange_halo()
+            if n >= sched.discard:
+                slab.slab_obs_partial()
+                slab.pcc_global.copy_(self.comm.all_reduce_sum(slab.pcc_partial.clone()))
+                slab.slab_pcc_feed()
+                if on_decision is not None and (n - sched.discard + 1) % sched.window == 0:
+                    on_decision(slab.pcc_get_state())
+        return slab.pcc_get_state()
+
     def measure(self):
         """observables of the whole lattice: the slabs' partial sums added over the ranks"""
         import torch

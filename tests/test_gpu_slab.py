@@ -93,3 +93,39 @@ def test_slab_errors(xy):
         import torch
         s.slab_flip(torch.zeros(2 * s.edges.numel(), dtype=torch.uint8, device="cuda"), 2, 0)   # no label phase yet
     s.destroy()
+
+
+@pytest.mark.parametrize("L,G", [(128, 2), (256, 4), (256, 1)])
+def test_sharded_pcc_equals_the_oracle_controller(xy, L, G):
+    """the PCC driver on G slabs: beta trace equal to the oracle's whole-lattice run, final angles bit for bit"""
+    from paper_1210_6116_b200 import shard
+    seed, n, window = 17, 240, 20
+    sg = xy.PccSchedule(n_sweeps=n, discard=20, window=window, dirs=1, dbeta0=1e-3, halve_every=100, dbeta_min=1e-6,
+                        target=2 / np.pi)
+    so = xo.PccSchedule(n_sweeps=n, discard=20, window=window, dirs=1, dbeta0=1e-3, halve_every=100, dbeta_min=1e-6,
+                        target=2 / np.pi)
+    ref_theta = xo.init(L, seed, xo.INIT_HOT)
+    ref = xo.pcc_run(ref_theta, L, seed, 0, 1.05, so, trace_cap=n)
+
+    def body(rank, comm):
+        rows, y_off = shard.slab_rows(L, G, rank)
+        slab = xy.SlabState(L, rows, y_off, seed, xy.INIT_HOT)
+        slab.set_obs_mode(xy.OBS_NONE)               # the sums come from xy_slab_obs_partial, once per sweep
+        return shard.ShardedLattice(slab, comm)
+    lats = shard.run_threads(G, body)
+    traces = [[] for _ in range(G)]
+
+    def run(rank, comm):
+        return lats[rank].pcc_run(1.05, sg, on_decision=lambda st: traces[rank].append(st.beta))
+    finals = shard.run_threads(G, run)
+    assert np.abs(ref["trace_bY"] - 2 / np.pi).min() > 1e-10          # no decision was a coin toss
+    # the controller's beta AFTER decision k is the beta the next window runs at
+    want_after = np.append(ref["trace_beta"][1:], ref["beta_final"])
+    for r in range(G):
+        assert finals[r].n_decisions == ref["n_decisions"] == (n - 20) // window
+        assert finals[r].beta == ref["beta_final"] and finals[r].dbeta == ref["dbeta_final"]
+        assert np.array_equal(np.array(traces[r]), want_after)
+    got = np.concatenate([lat.slab.get_angles() for lat in lats])
+    assert np.array_equal(got.view(np.uint32), ref_theta.view(np.uint32))
+    for lat in lats:
+        lat.slab.destroy()
