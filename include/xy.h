@@ -245,6 +245,9 @@ int xy_slab_create(xy_state **out, uint32_t L, uint32_t rows, uint32_t y_off, ui
  * last row: its +y bond) */
 int xy_slab_buffers(xy_state *s, void **dev_first_row, void **dev_halo_row, size_t *row_bytes, void **dev_edges, size_t *edge_bytes);
 int xy_slab_label(xy_state *s, double beta, void *cuda_stream);
+/* parity hook: the label phase on an injected bond set of the slab's sites (canonical bytes as xy_get_bonds); the
+ * following xy_slab_flip stitches (and flips with the coins of the current sweep counter) */
+int xy_slab_label_bonds(xy_state *s, const uint8_t *host_bonds, size_t n);
 /* dev_gathered_edges: nranks edge records in rank order (device memory) */
 int xy_slab_flip(xy_state *s, const void *dev_gathered_edges, uint32_t nranks, uint32_t rank, void *cuda_stream);
 /* The PCC driver on a sharded lattice (the paper's own use of its multi-GPU code, PAPER.md:62-66 at L >= 8192): the

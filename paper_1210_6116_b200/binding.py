@@ -121,6 +121,7 @@ _SIGS = {
     "xy_slab_create": [C.POINTER(_vp), C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint64, C.c_int, C.c_uint32, _vp, C.c_size_t],
     "xy_slab_buffers": [_vp, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(C.c_size_t), C.POINTER(_vp), C.POINTER(C.c_size_t)],
     "xy_slab_label": [_vp, C.c_double, _vp],
+    "xy_slab_label_bonds": [_vp, _vp, C.c_size_t],
     "xy_slab_flip": [_vp, _vp, C.c_uint32, C.c_uint32, _vp],
     "xy_slab_pcc_setup": [_vp, C.c_double, C.c_double, C.POINTER(PccSchedule)],
     "xy_slab_label_pcc": [_vp, _vp],
@@ -394,6 +395,10 @@ class SlabState(XYState):
     def _stream(self, stream):
         import torch
         return torch.cuda.current_stream().cuda_stream if stream is None else stream
+
+    def slab_label_bonds(self, bonds):
+        b = np.ascontiguousarray(bonds, np.uint8)
+        _check(_lib.xy_slab_label_bonds(self._h, b.ctypes.data, b.size))
 
     def slab_pcc_setup(self, beta0, sched: PccSchedule):
         _check(_lib.xy_slab_pcc_setup(self._h, beta0, sched.dbeta0, C.byref(sched)))

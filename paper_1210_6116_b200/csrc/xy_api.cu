@@ -1184,6 +1184,35 @@ static int slab_label_common(xy_state *s, double beta, int beta_from_ctl, void *
 
 int xy_slab_label(xy_state *s, double beta, void *cuda_stream) { return slab_label_common(s, beta, 0, cuda_stream); }
 
+/* parity hook (the slab counterpart of xy_label_bonds): label an injected bond set of the slab's sites */
+int xy_slab_label_bonds(xy_state *s, const uint8_t *host_bonds, size_t n)
+{
+    if (!s || !host_bonds) return fail(XY_ERR_ARG, "NULL argument");
+    if (!s->slab) return fail(XY_ERR_STATE, "not a slab");
+    if (n != s->N) return fail(XY_ERR_ARG, "n=%zu but the slab holds %llu sites", n, (unsigned long long)s->N);
+    if (s->slab_labelled) return fail(XY_ERR_STATE, "xy_slab_flip of the previous label phase is pending");
+    DeviceGuard g(s->device);
+    if (int rc = ensure_stage(s)) return rc;
+    for (uint64_t first = 0; first < s->N; first += kStageBytes) {
+        const uint64_t m = s->N - first < kStageBytes ? s->N - first : kStageBytes;
+        CUDA_TRY(cudaMemcpyAsync(s->stage, host_bonds + first, m, cudaMemcpyHostToDevice, s->stream));
+        k_bonds_pack<<<148 * 4, 256, 0, s->stream>>>(static_cast<const uint8_t *>(s->stage), s->bonds(), first / 4, m / 4);
+        CUDA_TRY(cudaStreamSynchronize(s->stream));
+    }
+    SweepArgs a = base_args(s);
+    set_direction(s, s->T, a);
+    a.beta = 0.0;
+    s->ker.label(a, s->stream);
+    s->ker.merge(a, s->stream);
+    k_slab_edges<<<(s->L + 255) / 256, 256, 0, s->stream>>>(static_cast<const uint32_t *>(s->labels()), s->bonds(), s->L,
+                                                           s->rows, s->y_off, s->edges());
+    CUDA_TRY(cudaGetLastError());
+    s->launches += 3;
+    s->pending = a;
+    s->slab_labelled = true;
+    return XY_OK;
+}
+
 /* ---- PCC on a sharded lattice: the controller runs replicated on every rank, fed with all-reduced sums ---- */
 int xy_slab_pcc_setup(xy_state *s, double beta0, double dbeta0, const xy_pcc_schedule *sc)
 {

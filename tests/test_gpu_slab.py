@@ -129,3 +129,39 @@ def test_sharded_pcc_equals_the_oracle_controller(xy, L, G):
     assert np.array_equal(got.view(np.uint32), ref_theta.view(np.uint32))
     for lat in lats:
         lat.slab.destroy()
+
+
+@pytest.mark.parametrize("L,G", [(128, 2), (256, 4), (192, 3), (512, 8)])
+def test_stitch_on_injected_bond_patterns(xy, L, G):
+    """the label phase + stitch on adversarial bond sets (a serpentine that crosses every cut L/2 times, combs, stripes,
+    wrap-only bonds, random densities): canonical labels of the G slabs equal the oracle's labels of the whole lattice"""
+    import xy_inputs
+    from paper_1210_6116_b200 import shard
+    rng = np.random.default_rng(L + G)
+    sets = [(k, xy_inputs.pattern_bonds(L, k)) for k in xy_inputs.BOND_PATTERNS]
+    v_serp = np.zeros((L, L), np.uint8)                   # a snake running along the columns: crosses every cut L times
+    v_serp[: L - 1, :] |= 2
+    for x in range(L - 1):
+        v_serp[L - 1 if x % 2 == 0 else 0, x] |= 1
+    sets.append(("v_serpentine", v_serp.ravel()))
+    sets += [(f"random{p}", (rng.random(L * L) < p).astype(np.uint8) | ((rng.random(L * L) < p).astype(np.uint8) << 1))
+             for p in (0.1, 0.3, 0.5, 0.7, 0.9)]
+
+    def body(rank, comm):
+        rows, y_off = shard.slab_rows(L, G, rank)
+        return shard.ShardedLattice(xy.SlabState(L, rows, y_off, 3, xy.INIT_HOT), comm)
+    lats = shard.run_threads(G, body)
+    for name, b in sets:
+        want = xo.label(b, L)[0]
+
+        def run(rank, comm, b=b):
+            lat = lats[rank]
+            rows, y_off = lat.slab.rows, lat.slab.y_off
+            lat.slab.slab_label_bonds(b[y_off * L: (y_off + rows) * L])
+            g = lat.comm.all_gather(lat.slab.edges)
+            lat.slab.slab_flip(g.reshape(-1), G, rank)
+            return lat.slab.get_labels()
+        got = np.concatenate(shard.run_threads(G, run))
+        assert (got == want).all(), name
+    for lat in lats:
+        lat.slab.destroy()
