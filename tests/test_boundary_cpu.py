@@ -82,3 +82,30 @@ def test_product_code_is_independent_of_the_oracle():
     osrc = open(os.path.join(ROOT, "oracle", "xy_oracle.c")).read()
     assert "cuda" not in re.sub(r"/\*.*?\*/", "", osrc, flags=re.S).lower()
     assert "#include \"" not in osrc                      # no project headers shared with the CUDA path
+
+
+def test_struct_layouts_match_the_header(tmp_path):
+    """sizeof / offsetof of every struct of include/xy.h as a C compiler sees them against the ctypes mirrors of the
+    binding (a silent mismatch would corrupt records without failing a call)."""
+    import subprocess
+    from paper_1210_6116_b200 import binding as b
+    pairs = {"xy_obs": b.Obs, "xy_fourier": b.Fourier, "xy_pcc_schedule": b.PccSchedule, "xy_pcc_out": b._PccOut,
+             "xy_pcc_state": b.PccState, "xy_potts_obs": b.PottsObs}
+    lines = ['#include <stdio.h>', '#include <stddef.h>', f'#include "{os.path.join(ROOT, "include", "xy.h")}"', 'int main(void) {']
+    for cname, cls in pairs.items():
+        lines.append(f'printf("{cname} %zu", sizeof({cname}));')
+        for fname, _ in cls._fields_:
+            lines.append(f'printf(" %zu", offsetof({cname}, {fname}));')
+        lines.append('printf("\\n");')
+    lines += ['return 0; }']
+    src = tmp_path / "layout.c"
+    src.write_text("\n".join(lines))
+    exe = tmp_path / "layout"
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", str(src), "-o", str(exe)], check=True)
+    out = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.strip().splitlines()
+    assert len(out) == len(pairs)
+    for line in out:
+        name, size, *offs = line.split()
+        cls = pairs[name]
+        assert int(size) == C.sizeof(cls), name
+        assert [int(o) for o in offs] == [getattr(cls, f).offset for f, _ in cls._fields_], name
