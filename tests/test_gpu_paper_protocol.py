@@ -1,7 +1,7 @@
 """The paper's PCC protocol on the GPU (beta*Upsilon against 0.636508 over windows of
 1000 MCS, dbeta = 5e-4, 60 000 MCS discarded), shortened to 3e5 measured sweeps, against Table I
-(PAPER.md:80-88): beta_KT(L), <m^2>_L and xi_2nd(L)/L for L = 64 ... 1024 by default (L = 2048 and 4096 with
-XY_LONG=1: 40 s and 80 s of GPU time).  Statistical pins with the error bar of THIS run: the beta trace is
+(PAPER.md:80-88): beta_KT(L), <m^2>_L and xi_2nd(L)/L for L = 64 ... 4096, all in the default run (L = 2048 and 4096
+take 40 s and 80 s of GPU time).  Statistical pins with the error bar of THIS run: the beta trace is
 binned into 10 blocks of 30 windows; <m^2> and chi(2 pi / L) come from the controller's device-side sums over ALL 3e5
 measured sweeps, read after each of ten chunks (xy_pcc_run + 9 x xy_pcc_continue), xi_2nd by jackknife over the ten
 blocks; a value passes if it is within 5 combined standard errors (ours and the
@@ -27,18 +27,13 @@ def xy():
     return m
 
 
-LONG = os.environ.get("XY_LONG") == "1"          # L = 1024 and 4096 take 20 s and 80 s of GPU time: opt-in
-
-
 def _within(name, value, err, paper, paper_err, cap):
     tol = 5.0 * float(np.hypot(err, paper_err))
     assert abs(value - paper) <= tol, f"{name}: {value} +- {err} vs paper {paper} +- {paper_err} (5 sigma = {tol})"
     assert abs(value - paper) <= cap, f"{name}: {value} vs paper {paper}: outside the cap {cap}"
 
 
-@pytest.mark.parametrize("L,seed", [(64, 21), (128, 22), (256, 25), (512, 26), (1024, 23),
-                                    pytest.param(2048, 27, marks=pytest.mark.skipif(not LONG, reason="set XY_LONG=1")),
-                                    pytest.param(4096, 24, marks=pytest.mark.skipif(not LONG, reason="set XY_LONG=1"))])
+@pytest.mark.parametrize("L,seed", [(64, 21), (128, 22), (256, 25), (512, 26), (1024, 23), (2048, 27), (4096, 24)])
 def test_paper_protocol_table1(xy, L, seed):
     row = table1()[L]
     c = constants()
