@@ -168,12 +168,18 @@ k_potts_flip(const SweepArgs a, const PottsArgs p)
     //      is a global root, else the root k_merge linked them to ----
     if (tid == 0) nqueue = 0;
     __syncthreads();
-    uint32_t rb = 0, ncl = 0;
+    uint32_t rb = 0, merged = 0, ncl = 0;             // root bits of my sites; of those, the ones k_merge linked elsewhere
 #pragma unroll
     for (int k = 0; k < NP; ++k) {
         const size_t i = (size_t)(y0 + k * RPP + rq) * L + x0 + 4 * q4;
+        LabelT lab[4];
+        load_labels(i, lab);                         // coalesced; read again (from L2) in the last phase
         rb |= ((__ldg(reinterpret_cast<const uint8_t *>(a.rootmask) + (i >> 3)) >> (i & 4u)) & 15u) << (4 * k);
+#pragma unroll
+        for (int v = 0; v < 4; ++v)
+            if (lab[v] != (LabelT)(i + v)) merged |= 1u << (4 * k + v);
     }
+    merged &= rb;
     {
         // one slot reservation per warp: ballots of the four-bit counts
         const uint32_t n = __popc(rb);
@@ -190,17 +196,19 @@ k_potts_flip(const SweepArgs a, const PottsArgs p)
         while (bits) {
             const int b = __ffs(bits) - 1;
             bits &= bits - 1;
-            queue[slot++] = (uint16_t)(((b >> 2) * RPP + rq) * TW + 4 * q4 + (b & 3));
+            // tile-local index (< 2^15) and, in bit 15, whether the root was linked elsewhere
+            queue[slot++] = (uint16_t)((((b >> 2) * RPP + rq) * TW + 4 * q4 + (b & 3)) | (((merged >> b) & 1u) << 15));
         }
     }
     __syncthreads();
     for (uint32_t j = tid; j < nqueue; j += NT) {
-        const uint32_t loc = queue[j];
+        const uint32_t e = queue[j], loc = e & 0x7fffu;
         const LabelT self = gbase + (LabelT)(loc / TW) * L + (loc % TW);
-        LabelT root = __ldg(labels + self);
-        if (root == self) {
+        LabelT root = self;
+        if (!(e & 0x8000u)) {
             ++ncl;
         } else {                                                         // read-only chase: the forest is final
+            root = __ldg(labels + self);
             LabelT up = __ldg(labels + root);
             while (up != root) { XY_CHECK(CHK_GLABEL, up < root); root = up; up = __ldg(labels + root); }
         }
