@@ -224,7 +224,7 @@ def timed_leg(xy, torch, L, init, seed, beta, flags=0, therm=0, warm=3, K=20, ob
     out = {"L": L, "init": init, "seed": seed, "beta": beta, "label_bytes": lb, "observables": obs, "untimed_sweeps": therm + warm,
            "steps": K, "ms_per_step": ms / K, "updates_per_s": N * K / (ms * 1e-3), "bytes_per_site": bps,
            "sweep_roofline_frac": bps * N * K / (ms * 1e-3) / 1e9 / peak,
-           "frac_on_survey_R0": (20.5 + 2 * lb) * N * K / (ms * 1e-3) / 1e9 / peak,
+           "frac_on_survey_R0": (12.5 + 4 * lb) * N * K / (ms * 1e-3) / 1e9 / peak,
            "bond_density": (o.n_bonds_x + o.n_bonds_y) / (2 * N), "clusters_per_site": o.n_clusters / N}
     if (4 + lb) * N < 4 * 126e6:
         out["note"] = "working set comparable to the 126 MB L2: not an HBM measurement"
@@ -606,9 +606,9 @@ def main():
             "sweep_roofline": {"bytes_per_site": sweep_bytes, "achieved_gbs": sweep_gbs, "frac": sweep_gbs / peak,
                                "floor_bytes_per_site": 8.0 + 2 * label_bytes,
                                # SURVEY.md 8(d)'s reference model R0 (five separate passes incl. a flatten pass this
-                               # design does not have): the same time against 28.5 / 44.5 B per site
-                               "survey_R0_bytes_per_site": 20.5 + 2 * label_bytes,
-                               "frac_on_survey_R0": (20.5 + 2 * label_bytes) * N * K / (ms * 1e-3) / 1e9 / peak,
+                               # design does not have): the same time against 12.5 + 4 w = 28.5 / 44.5 B per site
+                               "survey_R0_bytes_per_site": 12.5 + 4 * label_bytes,
+                               "frac_on_survey_R0": (12.5 + 4 * label_bytes) * N * K / (ms * 1e-3) / 1e9 / peak,
                                "ns_per_site": ms * 1e6 / (K * N)},
             "observables": {"sweep": int(obs.sweep), "E_per_site": obs.E / N,
                             "m2": (obs.Mx ** 2 + obs.My ** 2) / N ** 2,
