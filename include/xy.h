@@ -223,6 +223,32 @@ int xy_debug_curand_philox(const uint32_t *ctr_host, const uint32_t *key_host, u
  * all zeros from the normal build, which compiles the checks away. */
 int xy_debug_check_counts(uint64_t counts[8], int *checked_build);
 
+/* ---- observables without any allocation ------------------------------------------------------
+ * The sums E, Mx, My, Cx, Sx, Cy, Sy of xy_obs (PAPER.md:40 Eq. 3, :46-54 Eq. 4-6) of a configuration the CALLER holds
+ * in device memory, for programs in which this library may not allocate device memory: a host application that has
+ * handed the whole GPU to its own pool (a framework's caching allocator, a fixed per-job memory budget), so that a
+ * cudaMalloc from a library can fail or fragment it; and loops that cannot afford the device-wide stall a cudaMalloc /
+ * cudaFree implies while other streams are busy.  Every other way to these sums goes through a state, whose creation
+ * allocates or needs a workspace of 8.4 bytes per site.
+ *   dev_theta  in : L*L angles in DEVICE memory, row-major, each in [0, 6.2831855] as everywhere in this library
+ *                   (not checked here: an angle outside that range makes the kernel fault); not modified.
+ *   L             : a multiple of 64 with 64 <= L <= 65536; anything else is rejected with XY_ERR_UNSUPPORTED_L and
+ *                   nothing is launched.
+ *   dev_out    out: one xy_obs in DEVICE memory (8-byte aligned).  The seven sums are written; sweep, beta and the
+ *                   three counts read 0.  The sums are the ones xy_measure returns for the same angles on the same
+ *                   GPU (same kernel, same grid, same summation order).
+ *   cuda_stream   : the work (two small memsets and one kernel) is only ENQUEUED there; NULL = legacy default stream.
+ * Scratch: the per-CTA partial sums, the last-CTA ticket and the sine / cosine table sit in one file-scope device array
+ * of 406 528 bytes (under 0.4 MiB) that every GPU which loads this library carries until the process ends.  All calls
+ * on a device share it and find the previous call's contents in it; the call clears what has to start at zero.  Two
+ * calls whose kernels can overlap on one GPU (different streams, or two host threads) therefore RACE: serialise them.
+ * The first call on each device does the one-time set-up for that device (looks up the array's device address, uploads
+ * the 103 KB table with a blocking copy, sets kernel attributes, synchronises the device), so make that first call
+ * during start-up, on the device you will use, and before you begin any stream capture.
+ * The call uses no cudaMalloc, cudaFree or allocating library routine, before or after set-up.
+ * Errors: XY_ERR_ARG (NULL or non-device pointer), XY_ERR_UNSUPPORTED_L, XY_ERR_CUDA. */
+int xy_observe_static(const float *dev_theta, uint32_t L, xy_obs *dev_out, void *cuda_stream);
+
 /* ---- row-slab sharding across GPUs (SURVEY.md 8(e) / 8(f) #3; PAPER.md:34 "the inter-GPU labeling", :64) ----------
  * One state per rank holds rows [y_off, y_off + rows) of the L x L lattice (rows and y_off multiples of 32, fewer than
  * 2^31 sites, 32-bit labels) plus one halo row: the first row of the slab below (of rank 0 for the last rank).  Every

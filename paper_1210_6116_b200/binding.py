@@ -139,6 +139,7 @@ _SIGS = {
     "xy_potts_get_bonds": [_vp, _vp, C.c_size_t],
     "xy_potts_get_labels": [_vp, _vp, C.c_size_t],
     "xy_potts_get_launch_count": [_vp, C.POINTER(C.c_uint64)],
+    "xy_observe_static": [_vp, C.c_uint32, _vp, _vp],
     "xy_debug_philox": [_vp, _vp, _vp, C.c_size_t],
     "xy_debug_curand_philox": [_vp, _vp, _vp, C.c_size_t],
 }
@@ -331,6 +332,23 @@ class XYState:
     def label_bonds(self, bonds):
         b = np.ascontiguousarray(bonds, np.uint8)
         _check(_lib.xy_label_bonds(self._h, b.ctypes.data, self.N))
+
+
+def observe_static(theta, L, out=None, stream=None):
+    """xy_observe_static: the seven observable sums of the L x L angles in the CUDA tensor `theta` (float32, contiguous),
+    for callers whose device memory is all spoken for (a pool or caching allocator owns it, or a cudaMalloc would stall
+    busy streams): the kernel's scratch is a fixed array inside the library, so nothing is allocated on the device --
+    `out` included if the caller passes it (a CUDA uint8 tensor of sizeof(xy_obs) = 96 bytes; None: this wrapper makes
+    one with torch).  Only enqueues; returns `out`, readable as OBS_DTYPE after a synchronise.  Calls on one GPU share
+    the scratch and must not overlap; the first call per device does a blocking set-up (see include/xy.h)."""
+    import torch
+    assert theta.is_cuda and theta.dtype == torch.float32 and theta.is_contiguous() and theta.numel() == L * L
+    if out is None:
+        out = torch.empty(C.sizeof(Obs), dtype=torch.uint8, device=theta.device)
+    assert out.is_cuda and out.is_contiguous() and out.numel() * out.element_size() >= C.sizeof(Obs)
+    st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+    _check(_lib.xy_observe_static(theta.data_ptr(), L, out.data_ptr(), st))
+    return out
 
 
 def _philox_common(fn, ctr, key):

@@ -13,6 +13,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <limits>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1324,5 +1325,128 @@ int xy_debug_curand_philox(const uint32_t *ctr, const uint32_t *key, uint32_t *o
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// xy_observe_static: the observables-only pass of k_bonds for callers that must not allocate.
+//
+// k_bonds needs global memory beyond its input and output: one record of partial sums per CTA, the
+// last-CTA ticket, and the (cos, sin)(k / 1024) table.  A state carves these out of its workspace; here
+// they live in ONE file-scope device array that every GPU loading this library holds until the process
+// exits (kStaticScratchBytes, about 0.4 MB).  Nothing on this path calls cudaMalloc / cudaFree or a
+// library routine that allocates device memory.
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+constexpr size_t cx_align256(size_t v) { return (v + 255) / 256 * 256; }
+constexpr size_t kStaticOffPartials = 0;
+constexpr size_t kStaticOffTab = cx_align256(kStaticOffPartials + (size_t)kMaxGrid * kPartialStride * sizeof(double));
+constexpr size_t kStaticOffCtl = cx_align256(kStaticOffTab + (size_t)(kTabN + 1) * sizeof(double2));
+constexpr size_t kStaticScratchBytes = cx_align256(kStaticOffCtl + sizeof(DevCtl));
+static_assert(kStaticScratchBytes == 406528, "include/xy.h states this size");
+
+// In host code this name is only a handle for cudaGetSymbolAddress: it is NOT a device address.
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+constexpr int kStaticMaxDevices = 64;
+struct StaticDev {
+    bool ready = false;
+    unsigned char *base = nullptr;     // device address of g_static_scratch on this device
+    int sms = 0;
+    int occ[2][2] = {{0, 0}, {0, 0}};  // CTAs per SM of k_bonds<VEC, RS, false, true, false>: [VEC == 4][RS == kRSLarge]
+};
+StaticDev g_static_dev[kStaticMaxDevices];
+std::mutex g_static_mu;
+
+// once per device, with that device current: resolve the array's device address, upload the table, opt the
+// four kernel variants in to their shared memory, query their occupancy, zero the control block
+int static_setup(int dev, StaticDev &d)
+{
+    unsigned char *p = nullptr;
+    CUDA_TRY(cudaGetSymbolAddress((void **)&p, g_static_scratch));
+    if (!p || ((uintptr_t)p & 255u)) return fail(XY_ERR_CUDA, "static scratch has no usable device address");
+    {
+        std::vector<double2> h(kTabN + 1);
+        for (int k = 0; k <= kTabN; ++k) {
+            const long double ang = (long double)k / 1024.0L;
+            h[k].x = (double)cosl(ang);
+            h[k].y = (double)sinl(ang);
+        }
+        CUDA_TRY(cudaMemcpy(p + kStaticOffTab, h.data(), h.size() * sizeof(double2), cudaMemcpyHostToDevice));
+    }
+    CUDA_TRY(cudaMemset(p + kStaticOffCtl, 0, sizeof(DevCtl)));
+    CUDA_TRY((KS<2, kR, kNW, kRSSmall, uint32_t>::bonds_prepare<false, true, false>(&d.occ[0][0])));
+    CUDA_TRY((KS<2, kR, kNW, kRSLarge, uint32_t>::bonds_prepare<false, true, false>(&d.occ[0][1])));
+    CUDA_TRY((KS<4, kR, kNW, kRSSmall, uint32_t>::bonds_prepare<false, true, false>(&d.occ[1][0])));
+    CUDA_TRY((KS<4, kR, kNW, kRSLarge, uint32_t>::bonds_prepare<false, true, false>(&d.occ[1][1])));
+    CUDA_TRY(cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev));
+    for (int v = 0; v < 2; ++v)
+        for (int r = 0; r < 2; ++r)
+            if (d.occ[v][r] < 1) return fail(XY_ERR_CUDA, "k_bonds does not fit this GPU (was the library built for sm_100a?)");
+    CUDA_TRY(cudaDeviceSynchronize());
+    d.base = p;
+    d.ready = true;
+    return XY_OK;
+}
+
+int is_device_pointer(const void *p)
+{
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+}  // namespace
+
+extern "C" int xy_observe_static(const float *dev_theta, uint32_t L, xy_obs *dev_out, void *cuda_stream)
+{
+    if (!dev_theta || !dev_out) return fail(XY_ERR_ARG, "NULL argument");
+    if (L > 65536)
+        return fail(XY_ERR_UNSUPPORTED_L, "L=%u unsupported: xy_observe_static handles lattices up to 65536 x 65536 (a multiple of 64)", L);
+    if (int rc = check_L(L)) return rc;
+    if (!is_device_pointer(dev_theta) || !is_device_pointer(dev_out))
+        return fail(XY_ERR_ARG, "dev_theta and dev_out must be device memory");
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return fail(XY_ERR_CUDA, "device ordinal %d not supported (limit %d)", dev, kStaticMaxDevices);
+    StaticDev &d = g_static_dev[dev];
+    {
+        std::lock_guard<std::mutex> lock(g_static_mu);
+        if (!d.ready)
+            if (int rc = static_setup(dev, d)) return rc;
+    }
+    const bool vec4 = L % 128 == 0, large = L > 4096;
+    const int rs = large ? kRSLarge : kRSSmall;
+    const uint32_t nstrips = (L / (vec4 ? 128u : 64u)) * (L / (uint32_t)rs);
+    // the grid of a state's k_bonds with observables (create_common): same partial sums in the same order
+    long need = (nstrips + BondsShape<true>::warps - 1) / BondsShape<true>::warps;
+    long g = (long)d.sms * d.occ[vec4][large];
+    if (g > need) g = need;
+    if (g > (long)kMaxGrid) g = kMaxGrid;
+
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    SweepArgs a;
+    memset(&a, 0, sizeof a);
+    a.theta = const_cast<float *>(dev_theta);            // the observables-only variant never writes theta
+    a.partials = reinterpret_cast<double *>(d.base + kStaticOffPartials);
+    a.sincos_tab = reinterpret_cast<const double2 *>(d.base + kStaticOffTab);
+    a.ctl = reinterpret_cast<DevCtl *>(d.base + kStaticOffCtl);
+    a.ring = dev_out;                                    // ring of one record: record t % 1 = 0 is the caller's
+    a.ring_cap = 1;
+    a.L = L;
+    a.rows = L;
+    a.obs_fill = 1;
+    a.cphi = 1.0;                                        // unrotated frame (phi = 0), as xy_measure
+    // what must start at zero: the last-CTA ticket (left non-zero by a launch that did not finish) and the
+    // fields of the record the kernel does not write; the partial sums are overwritten before they are read
+    CUDA_TRY(cudaMemsetAsync(a.ctl, 0, sizeof(DevCtl), st));
+    CUDA_TRY(cudaMemsetAsync(dev_out, 0, sizeof(xy_obs), st));
+    cudaError_t e;
+    if (vec4) e = large ? KS<4, kR, kNW, kRSLarge, uint32_t>::bonds_launch<false, true, false>(a, (int)g, st)
+                        : KS<4, kR, kNW, kRSSmall, uint32_t>::bonds_launch<false, true, false>(a, (int)g, st);
+    else e = large ? KS<2, kR, kNW, kRSLarge, uint32_t>::bonds_launch<false, true, false>(a, (int)g, st)
+                   : KS<2, kR, kNW, kRSSmall, uint32_t>::bonds_launch<false, true, false>(a, (int)g, st);
+    CUDA_TRY(e);
+    return XY_OK;
+}
 
 #include "potts_api.cuh"
