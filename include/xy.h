@@ -183,12 +183,19 @@ int xy_series_capacity(xy_state *s, uint64_t *cap);
  * as the device ring still holds them (same window as xy_get_series).  out / host: HOST memory. */
 int xy_measure_fourier(xy_state *s, xy_fourier *out);
 int xy_get_fourier_series(xy_state *s, xy_fourier *host, uint64_t first_sweep, uint64_t count);
+/* Second-moment correlation length (Eq. 8) from chi(0) and chi(2 pi / L) of Eq. 9:
+ *   *out = sqrt(chi0 / chik - 1) / (2 sin(pi / L)).
+ * chi0 = <Mx^2 + My^2> / N and chik = <|Fx|^2 + |Fy|^2> / (2 N) are the caller's averages over measured sweeps (xy_obs and
+ * xy_fourier records, or N * sum_m2 / n_acc and sum_chik / n_acc of xy_pcc_state).  Host arithmetic on two numbers; no
+ * state, no GPU.  XY_ERR_ARG (and *out = NaN) unless L >= 2, chik > 0 and chi0 >= chik, all finite. */
+int xy_xi2nd(double chi0, double chik, uint32_t L, double *out);
 int xy_get_sweep(xy_state *s, uint64_t *t);
 int xy_set_sweep(xy_state *s, uint64_t t);                      /* resume / sampled-sweep parity */
 int xy_debug_fix_phi(xy_state *s, int on, double phi);          /* Ising-limit and 2x2-style tests */
 /* XY_OBS_NONE: the following xy_sw_sweeps (and the `discard` sweeps of xy_pcc_run) skip the fp64
  * observable sums (the bond decisions, labels and angles are unchanged, bit for bit); their ring records
- * keep beta and the counts, the sums read NaN.  xy_measure still returns the sums of the current
+ * keep beta and the counts, the sums read NaN (so do the xy_fourier records of those sweeps, with their sweep
+ * number set).  xy_measure still returns the sums of the current
  * configuration (one observables-only pass).  XY_OBS_ALL (default) restores the per-sweep series. */
 int xy_set_obs_mode(xy_state *s, int mode);
 /* number of bond decisions of all sweeps so far that the fp32 filter could not settle and that
@@ -251,7 +258,7 @@ int xy_observe_static(const float *dev_theta, uint32_t L, xy_obs *dev_out, void 
 
 /* ---- row-slab sharding across GPUs (SURVEY.md 8(e) / 8(f) #3; PAPER.md:34 "the inter-GPU labeling", :64) ----------
  * One state per rank holds rows [y_off, y_off + rows) of the L x L lattice (rows and y_off multiples of 32, fewer than
- * 2^31 sites, 32-bit labels) plus one halo row: the first row of the slab below (of rank 0 for the last rank).  Every
+ * 2^31 sites -- L = 65536 therefore needs at least 4 slabs --, 32-bit labels) plus one halo row: the first row of the slab below (of rank 0 for the last rank).  Every
  * random number is keyed by the site's index in the WHOLE lattice, so G slabs reproduce the sweep of one L x L state
  * bit for bit.  One sweep at counter t is
  *     xy_slab_label   (every rank)  direction, bonds, local labels (tile labeling + merge inside the slab), edge record
@@ -260,6 +267,9 @@ int xy_observe_static(const float *dev_theta, uint32_t L, xy_obs *dev_out, void 
  *     exchange of first rows -> halo rows (caller), before the next xy_slab_label or xy_measure.
  * xy_measure / xy_get_series return the slab's PARTIAL sums (its sites; the y links of its last row use the halo row;
  * n_clusters counts the clusters whose canonical root lies in the slab): the caller adds the ranks' records.
+ * The halo row is valid from creation (cold: zeros; hot: the initial values of that row of the whole lattice).  Edge sites
+ * of this rank's gathered record that lie outside the slab (wrong rank / nranks, records out of rank order) are skipped
+ * by xy_slab_flip and reported as XY_ERR_ARG by the next xy_measure or xy_get_labels of the slab.
  * xy_get_labels returns canonical labels of the whole lattice (after xy_slab_flip).  xy_sw_sweeps, xy_pcc_run,
  * xy_label_bonds and xy_debug_check_labels return XY_ERR_STATE on a slab. */
 int xy_slab_workspace_bytes(uint32_t L, uint32_t rows, uint32_t flags, size_t *nbytes);

@@ -9,7 +9,7 @@ library) can be imported before the library exists.
 """
 __all__ = ["XYState", "XYError", "Obs", "PccSchedule", "OBS_DTYPE", "INIT_COLD", "INIT_HOT", "OBS_NONE", "OBS_ALL",
            "FLAG_LABELS64", "FLAG_FOURIER", "Fourier", "FOURIER_DTYPE", "workspace_bytes", "debug_philox", "debug_check_counts", "debug_curand_philox", "lib_path",
-           "PottsState", "PottsObs", "SlabState", "PccState", "observe_static"]
+           "PottsState", "PottsObs", "SlabState", "PccState", "observe_static", "xi2nd"]
 
 
 def __getattr__(name):

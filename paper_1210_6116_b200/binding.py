@@ -140,6 +140,7 @@ _SIGS = {
     "xy_potts_get_labels": [_vp, _vp, C.c_size_t],
     "xy_potts_get_launch_count": [_vp, C.POINTER(C.c_uint64)],
     "xy_observe_static": [_vp, C.c_uint32, _vp, _vp],
+    "xy_xi2nd": [C.c_double, C.c_double, C.c_uint32, C.POINTER(C.c_double)],
     "xy_debug_philox": [_vp, _vp, _vp, C.c_size_t],
     "xy_debug_curand_philox": [_vp, _vp, _vp, C.c_size_t],
 }
@@ -332,6 +333,13 @@ class XYState:
     def label_bonds(self, bonds):
         b = np.ascontiguousarray(bonds, np.uint8)
         _check(_lib.xy_label_bonds(self._h, b.ctypes.data, self.N))
+
+
+def xi2nd(chi0, chik, L):
+    """xy_xi2nd: PAPER.md Eq. 8 from the averaged chi(0) and chi(2 pi / L)"""
+    out = C.c_double()
+    _check(_lib.xy_xi2nd(chi0, chik, L, C.byref(out)))
+    return out.value
 
 
 def observe_static(theta, L, out=None, stream=None):

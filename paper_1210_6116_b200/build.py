@@ -12,6 +12,7 @@ LIB = os.path.join(HERE, "libxy_b200.so")
 SOURCES = [os.path.join(CSRC, "xy_api.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "xy_kernels.cuh"), os.path.join(CSRC, "xy_device.cuh"),
                   os.path.join(CSRC, "potts_kernels.cuh"), os.path.join(CSRC, "potts_api.cuh"),
+                  os.path.join(CSRC, "slab_kernels.cuh"),
                   os.path.join(HERE, "..", "include", "xy.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-Wall", "-shared"]

@@ -104,13 +104,14 @@ __global__ void k_stitch_union(StitchTable t, const unsigned char *gathered, uin
 
 // my own edge sites: override the local root's label entry where the cluster's canonical root lies elsewhere
 __global__ void k_stitch_apply(StitchTable t, const unsigned char *gathered, uint32_t L, uint32_t rank, uint32_t y_off,
-                               uint32_t *labels, uint64_t *xroot)
+                               uint64_t nsites, uint32_t *labels, uint64_t *xroot, unsigned int *bad)
 {
     const size_t rb = slab_edge_bytes(L);
     const uint64_t goff = (uint64_t)y_off * L;
     const uint64_t *mine = reinterpret_cast<const uint64_t *>(gathered + (size_t)rank * rb);
     for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < 2u * L; j += gridDim.x * blockDim.x) {
         const uint64_t k = mine[j];
+        if (k - goff >= nsites) { atomicAdd(bad, 1u); continue; }    // not a site of this slab: the record is not this rank's
         if (j != 0 && j != L && mine[j - 1] == k) continue;          // the left neighbour does the same
         const uint32_t root = stitch_find(t, t.slot_of[rank * 2u * L + j]);
         const uint64_t g = t.key[root];

@@ -282,7 +282,6 @@ struct xy_state {
     Kernels ker{};
     int grid_bonds = 0, grid_bonds_noobs = 0, grid_fl = 0;
     int obs_mode = XY_OBS_ALL;      // xy_set_obs_mode
-    bool poisoned = false;          // xy_set_angles rejected its input and nothing valid was restored
     cudaStream_t stream = nullptr;
     bool have_sweep = false;        // bonds / labels of a sweep exist
     bool labels_flat = false;
@@ -370,7 +369,7 @@ SweepArgs base_args(const xy_state *s)
     a.t = (uint32_t)s->T;
     a.cphi = 1.0;                   // observables-only launches use the unrotated frame (phi = 0)
     a.sincos_tab = s->tab();
-    a.fring = s->fring();
+    a.fring = s->fourier() ? s->fring() : nullptr;
     {
         const long double ang = 6.283185307179586476925286766559L / (long double)s->L;
         a.ck1 = (double)cosl(ang);
@@ -415,6 +414,19 @@ int ensure_obs(xy_state *s, int feed_pcc)
     s->launches += 1;
     s->obs_valid_T = s->T;
     return XY_OK;
+}
+
+// slab: did an earlier xy_slab_flip meet edge records that were not this rank's (k_stitch_apply skipped them)?  Blocking.
+int slab_stitch_check(xy_state *s)
+{
+    if (!s->slab) return XY_OK;
+    unsigned int bad = 0;
+    CUDA_TRY(cudaMemcpyAsync(&bad, &s->ctl()->stitch_bad, sizeof bad, cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    if (!bad) return XY_OK;
+    CUDA_TRY(cudaMemsetAsync(&s->ctl()->stitch_bad, 0, sizeof bad, s->stream));
+    return fail(XY_ERR_ARG, "xy_slab_flip: %u edge sites of the gathered record of this rank lie outside the slab "
+                            "(wrong rank or nranks, or records not in rank order); the labels of that sweep are not valid", bad);
 }
 
 constexpr size_t kTimedSweepsPerFlush = 1024;
@@ -593,6 +605,10 @@ static int create_common(xy_state **out, uint32_t L, uint32_t rows, uint32_t y_o
         e = cudaMemsetAsync(s->theta(), 0, (s->N + (slab ? L : 0)) * 4, nullptr);
     } else {
         k_init_hot<<<148 * 8, 256>>>(s->theta(), s->N, (uint64_t)y_off * L, (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32));
+        // halo row of a slab: the initial values of the row below it in the whole lattice (the draws are keyed by the
+        // global site index), so the slab is complete before the caller's first exchange
+        if (slab) k_init_hot<<<(L + 255) / 256, 256>>>(s->theta() + s->N, L, (uint64_t)((y_off + rows) % L) * L,
+                                                       (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32));
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) {
@@ -683,7 +699,7 @@ int xy_measure(xy_state *s, xy_obs *out)
     if (int rc = ensure_obs(s, 0)) return rc;
     CUDA_TRY(cudaMemcpyAsync(out, s->ring() + (s->T % kRingCap), sizeof(xy_obs), cudaMemcpyDeviceToHost, s->stream));
     CUDA_TRY(cudaStreamSynchronize(s->stream));
-    return XY_OK;
+    return slab_stitch_check(s);
 }
 
 static int pcc_loop(xy_state *s, double beta0, double dbeta0, const xy_pcc_schedule *sc, xy_pcc_out *out, bool fresh)
@@ -821,6 +837,7 @@ int xy_set_angles(xy_state *s, const float *host, size_t n)
 {
     if (!s || !host) return fail(XY_ERR_ARG, "NULL argument");
     if (n != s->N) return fail(XY_ERR_ARG, "n=%zu but L*L=%llu", n, (unsigned long long)s->N);
+    if (s->slab_labelled) return fail(XY_ERR_STATE, "xy_slab_flip is pending: its labels live where the angles would be staged");
     DeviceGuard g(s->device);
     // staged in the label array (>= 4 N bytes; the labels of the previous sweep are given up), checked
     // there, and copied to theta only if every value is in range: a rejected call leaves theta untouched
@@ -944,6 +961,16 @@ int xy_get_fourier_series(xy_state *s, xy_fourier *host, uint64_t first, uint64_
     return XY_OK;
 }
 
+int xy_xi2nd(double chi0, double chik, uint32_t L, double *out)
+{
+    if (!out) return fail(XY_ERR_ARG, "out is NULL");
+    *out = std::numeric_limits<double>::quiet_NaN();
+    if (L < 2 || !std::isfinite(chi0) || !std::isfinite(chik) || !(chik > 0.0) || !(chi0 >= chik))
+        return fail(XY_ERR_ARG, "xi_2nd needs L >= 2 and finite chi(0) >= chi(2 pi / L) > 0");
+    *out = std::sqrt(chi0 / chik - 1.0) / (2.0 * std::sin(kPi / (double)L));
+    return XY_OK;
+}
+
 int xy_debug_check_counts(uint64_t counts[8], int *checked_build)
 {
     if (!counts || !checked_build) return fail(XY_ERR_ARG, "NULL argument");
@@ -993,6 +1020,7 @@ int xy_get_labels_range(xy_state *s, int64_t *host, uint64_t first, size_t n)
     if (s->slab) {
         // canonical labels of the whole lattice; valid after xy_slab_flip (the stitch overrides are in place)
         if (s->slab_labelled) return fail(XY_ERR_STATE, "labels of a slab are complete after xy_slab_flip");
+        if (int rc = slab_stitch_check(s)) return rc;
         const uint64_t chunk = kStageBytes / sizeof(int64_t);
         for (uint64_t done = 0; done < n; done += chunk) {
             const uint64_t m = n - done < chunk ? n - done : chunk;
@@ -1301,8 +1329,9 @@ int xy_slab_flip(xy_state *s, const void *dev_gathered_edges, uint32_t nranks, u
     k_stitch_clear<<<grid, 256, 0, s->stream>>>(s->stitch);
     k_stitch_insert<<<grid, 256, 0, s->stream>>>(s->stitch, gathered, s->L, nranks);
     k_stitch_union<<<grid, 256, 0, s->stream>>>(s->stitch, gathered, s->L, nranks);
-    k_stitch_apply<<<(2 * s->L + 255) / 256, 256, 0, s->stream>>>(s->stitch, gathered, s->L, rank, s->y_off,
-                                                                 static_cast<uint32_t *>(s->labels()), s->xroot());
+    k_stitch_apply<<<(2 * s->L + 255) / 256, 256, 0, s->stream>>>(s->stitch, gathered, s->L, rank, s->y_off, s->N,
+                                                                 static_cast<uint32_t *>(s->labels()), s->xroot(),
+                                                                 &s->ctl()->stitch_bad);
     s->ker.flip_slab(s->pending, s->stream);
     CUDA_TRY(cudaGetLastError());
     s->launches += 5;

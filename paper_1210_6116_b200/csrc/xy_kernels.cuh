@@ -50,6 +50,10 @@ struct DevCtl {
     // reading the per-sweep ring back
     double   sum_m2, sum_chik;
     unsigned long long n_acc;
+    // slab: edge sites of the gathered record that name a root outside this slab (wrong rank / order of the gather);
+    // k_stitch_apply skips them and counts them here, the next blocking call of the slab reports XY_ERR_ARG
+    unsigned int stitch_bad;
+    unsigned int pad2;
 };
 
 struct SweepArgs {
@@ -74,7 +78,7 @@ struct SweepArgs {
     double       phi, cphi, sphi, A;
     const double2 *sincos_tab;    // [kTabN + 1] (cos, sin)(k / 1024), host-computed
     double       ck1, sk1;        // (cos, sin)(2 pi / L)
-    xy_fourier  *fring;           // ring of structure-factor records (XY_FLAG_FOURIER), else unused
+    xy_fourier  *fring;           // ring of structure-factor records (XY_FLAG_FOURIER), else NULL
     // slab of a lattice sharded by rows: the state holds rows [y_off, y_off + rows) of the
     // L x L lattice; rows == L, y_off == 0, open_y == 0 for a whole lattice
     uint32_t     rows, y_off;
@@ -586,6 +590,11 @@ k_bonds(const SweepArgs a)
                 const double qnan = __longlong_as_double(0x7ff8000000000000LL);
                 o->E = qnan; o->Mx = qnan; o->My = qnan; o->Cx = qnan; o->Sx = qnan; o->Cy = qnan; o->Sy = qnan;
                 o->n_bonds_x = b0; o->n_bonds_y = b1; o->n_clusters = 0;
+                if (a.fring) {                                   // XY_FLAG_FOURIER: the same for the structure-factor record of T = t+1
+                    xy_fourier *f = a.fring + ((a.t + 1u) % a.ring_cap);
+                    f->sweep = (uint64_t)a.t + 1u;
+                    for (int k = 0; k < 4; ++k) { f->Fx[k] = qnan; f->Fy[k] = qnan; }
+                }
             }
             a.ctl->ticket = 0;
             __threadfence();

@@ -2,8 +2,8 @@
 
 Rank r of G holds rows [r L/G, (r+1) L/G) of the L x L lattice as one slab state (include/xy.h, "row-slab sharding").
 One sweep = local phase (direction, bonds, labels inside the slab, edge record) -> ALL-GATHER of the edge records
-(17 L bytes per rank) -> stitch + flip on every rank -> all-gather of the slabs' first rows (4 L bytes per rank), of
-which each rank keeps its lower neighbour's as its halo row.  Observables are partial sums per slab; `measure` adds
+(17 L bytes per rank, into a buffer allocated once) -> stitch + flip on every rank -> every rank sends its first row
+(4 L bytes) to its upper neighbour, whose halo row it is.  Observables are partial sums per slab; `measure` adds
 them with one all-reduce.  This module is plumbing only: every step of the path runs in the kernels behind the slab
 state; the transport is whatever `comm` wraps (torch.distributed with NCCL on the GPUs, gloo in the CPU test of this
 logic, threads of one process for the single-GPU parity test).
@@ -23,21 +23,39 @@ def slab_rows(L, world, rank):
 
 
 class DistComm:
-    """torch.distributed (backend nccl on the GPUs, gloo on CPU tensors)"""
+    """torch.distributed (backend nccl on the GPUs, gloo on CPU tensors).  The gathered buffers are allocated once per
+    (shape, dtype, device) and reused by every sweep; the halo row travels point to point (only the lower neighbour's
+    first row is needed), not through an all-gather."""
 
     def __init__(self, dist, rank, world):
         self.dist, self.rank, self.world = dist, rank, world
+        self._gathered = {}
 
     def all_gather(self, t):
+        """[world, *t.shape]; the returned tensor is this object's buffer and is overwritten by the next call with the
+        same shape"""
         import torch
         t = t.contiguous()
-        out = [torch.empty_like(t) for _ in range(self.world)]
-        self.dist.all_gather(out, t)
-        return torch.stack(out)
+        key = (tuple(t.shape), t.dtype, t.device)
+        out = self._gathered.get(key)
+        if out is None:
+            out = self._gathered[key] = torch.empty(self.world * t.numel(), dtype=t.dtype, device=t.device)
+        self.dist.all_gather_into_tensor(out, t.reshape(-1))      # flat in, flat out: what gloo and nccl both accept
+        return out.view((self.world,) + tuple(t.shape))
 
     def all_reduce_sum(self, t):
         self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM)
         return t
+
+    def shift_up(self, send, recv):
+        """recv <- the `send` of rank + 1 (periodic): every rank sends to rank - 1 and receives from rank + 1"""
+        if self.world == 1:
+            recv.copy_(send)
+            return
+        d = self.dist
+        ops = [d.P2POp(d.isend, send, (self.rank - 1) % self.world), d.P2POp(d.irecv, recv, (self.rank + 1) % self.world)]
+        for w in d.batch_isend_irecv(ops):
+            w.wait()
 
 
 class ThreadComm:
@@ -62,6 +80,15 @@ class ThreadComm:
     def all_reduce_sum(self, t):
         return self.all_gather(t).sum(dim=0)
 
+    def shift_up(self, send, recv):
+        self.s.slots[self.rank] = send
+        self.s.barrier.wait()
+        recv.copy_(self.s.slots[(self.rank + 1) % self.world])
+        if recv.is_cuda:
+            import torch
+            torch.cuda.current_stream().synchronize()   # the copy has read the neighbour's row before it may sweep on
+        self.s.barrier.wait()
+
 
 class ShardedLattice:
     """One rank's part of the sharded lattice.  `slab` is a SlabState (or, in the CPU test of this logic, an object with
@@ -73,8 +100,7 @@ class ShardedLattice:
         self.exchange_halo()
 
     def exchange_halo(self):
-        rows = self.comm.all_gather(self.slab.first_row)
-        self.slab.halo_row.copy_(rows[(self.rank + 1) % self.world])
+        self.comm.shift_up(self.slab.first_row, self.slab.halo_row)
 
     def sweep(self, beta, n=1):
         for _ in range(n):
@@ -96,7 +122,10 @@ class ShardedLattice:
             self.exchange_halo()
             if n >= sched.discard:
                 slab.slab_obs_partial()
-                slab.pcc_global.copy_(self.comm.all_reduce_sum(slab.pcc_partial.clone()))
+                slab.pcc_global.copy_(slab.pcc_partial)
+                total = self.comm.all_reduce_sum(slab.pcc_global)       # in place with torch.distributed
+                if total is not slab.pcc_global:
+                    slab.pcc_global.copy_(total)
                 slab.slab_pcc_feed()
                 if on_decision is not None and (n - sched.discard + 1) % sched.window == 0:
                     on_decision(slab.pcc_get_state())

@@ -1,4 +1,7 @@
-"""Workload for compute-sanitizer (memcheck / racecheck / synccheck) and for the range-checked build
+"""NOT a pytest (nothing collects it): the driver script of the range-checked build, run by hand as
+profiles/r2_checked_build.md states.
+
+Workload for compute-sanitizer (memcheck / racecheck / synccheck) and for the range-checked build
 (XY_NVCC_EXTRA=-DXY_CHECKED python -m paper_1210_6116_b200.build), kept small on purpose:
 
     compute-sanitizer --tool memcheck  python tests/sanitizer_driver.py

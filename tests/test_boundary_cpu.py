@@ -57,6 +57,26 @@ def test_workspace_bytes_and_argument_errors(lib):
     assert lib.xy_workspace_bytes(64, 0, None) == -1
 
 
+def test_xi2nd_is_eq8(lib):
+    """xy_xi2nd (host arithmetic, no GPU): Eq. 8 against closed forms -- an Ornstein-Zernike propagator
+    chi(k) = A / (xi^-2 + 4 sin^2(k/2)) returns its own xi exactly -- and against Table I's row L = 64 through the
+    oracle-free inversion chi0 / chik = 1 + (2 sin(pi/L) xi)^2"""
+    import math
+    lib.xy_xi2nd.argtypes = [C.c_double, C.c_double, C.c_uint32, C.POINTER(C.c_double)]
+    out = C.c_double()
+    for L in (64, 4096, 65536):
+        for xi in (0.3 * L, 0.7506912 * L, 5.0):
+            khat2 = 4.0 * math.sin(math.pi / L) ** 2
+            chi0, chik = 1.0 / xi ** -2, 1.0 / (xi ** -2 + khat2)
+            assert lib.xy_xi2nd(chi0, chik, L, C.byref(out)) == 0
+            assert out.value == pytest.approx(xi, rel=1e-9)
+    assert lib.xy_xi2nd(1.0, 0.0, 64, C.byref(out)) == -1 and math.isnan(out.value)
+    assert lib.xy_xi2nd(1.0, 2.0, 64, C.byref(out)) == -1
+    assert lib.xy_xi2nd(float("nan"), 1.0, 64, C.byref(out)) == -1
+    assert lib.xy_xi2nd(2.0, 1.0, 1, C.byref(out)) == -1
+    assert lib.xy_xi2nd(2.0, 1.0, 64, None) == -1
+
+
 def test_no_cpu_fallback(lib):
     """without a CUDA device xy_create must fail loudly, never compute on the host."""
     import torch

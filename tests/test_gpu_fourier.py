@@ -77,6 +77,35 @@ def test_fourier_series_along_sweeps(xy, L, flags):
     plain.destroy()
 
 
+def test_fourier_records_of_sweeps_without_observables_read_nan(xy):
+    """XY_OBS_NONE sweeps of a FOURIER state: their structure-factor records carry the sweep number and NaN sums (never
+    a stale record of an older sweep), the records around them are the oracle's, the chain itself is unchanged"""
+    L, seed, beta = 128, 9, 1.1
+    st = xy.XYState(L, seed, xy.INIT_HOT, flags=xy.FLAG_FOURIER)
+    ref = xo.init(L, seed, xo.INIT_HOT)
+    thetas = [ref.copy()]
+    for t in range(7):
+        xo.sweep(ref, L, seed, t, beta)
+        thetas.append(ref.copy())
+    st.sw_sweeps(beta, 3)                              # records 0..2 filled by the sweeps, 3 still open
+    st.set_obs_mode(xy.OBS_NONE)
+    st.sw_sweeps(beta, 2)                              # sweeps 3, 4: no sums; records 3 (incoming state of sweep 3) and 4 never filled
+    st.set_obs_mode(xy.OBS_ALL)
+    st.sw_sweeps(beta, 2)                              # sweeps 5, 6 fill records 5, 6; record 7 on demand
+    assert (st.get_angles() == ref).all()
+    ser = st.get_fourier_series(0, 8)
+    assert list(ser["sweep"]) == list(range(8))
+    for t in range(8):
+        F = np.concatenate([ser["Fx"][t], ser["Fy"][t]])
+        if t in (3, 4):
+            assert np.isnan(F).all(), (t, F)
+        else:
+            check_fourier(F, thetas[t], L, f"T={t}")
+    obs = st.get_series(0, 8)
+    assert np.isnan(obs["E"][3]) and np.isnan(obs["E"][4]) and not np.isnan(obs["E"][[0, 1, 2, 5, 6, 7]]).any()
+    st.destroy()
+
+
 def test_fourier_needs_flag(xy):
     st = xy.XYState(64, 1, xy.INIT_COLD)
     with pytest.raises(xy.XYError):

@@ -70,8 +70,9 @@ def test_paper_protocol_table1(xy, L, seed):
     m2 = m2s.mean()
     m2_err = m2s.std(ddof=1) / np.sqrt(nb)
     _within("<m^2>", m2, m2_err, row["m2"], row["m2_err"], 0.005)
-    xi_over_L = xo.xi2nd(N * m2, fks.mean(), L) / L
-    jk = np.array([xo.xi2nd(N * np.delete(m2s, b).mean(), np.delete(fks, b).mean(), L) / L for b in range(nb)])
+    xi_over_L = xy.xi2nd(N * m2, fks.mean(), L) / L          # Eq. 8 through the library (xy_xi2nd) ...
+    assert xi_over_L == pytest.approx(xo.xi2nd(N * m2, fks.mean(), L) / L, rel=1e-14)   # ... and the oracle's restatement
+    jk = np.array([xy.xi2nd(N * np.delete(m2s, b).mean(), np.delete(fks, b).mean(), L) / L for b in range(nb)])
     xi_err = np.sqrt((nb - 1) / nb * ((jk - jk.mean()) ** 2).sum())
     _within("xi_2nd/L", xi_over_L, xi_err, row["xi"], row["xi_err"], 0.012)
     # the device-side sums agree with the records the ring still holds (the last sweeps of the walk)
