@@ -1,13 +1,14 @@
 """Parity at the BASELINE configs' own sizes and schedules (north_star: bit-exact at every config), and the
 kernel variants that only large or odd sizes select.  Everything goes through the C-ABI.
 
-config 2 (L = 1024, cold, seed 7, beta in {0.90, 1.00, 1.12, 1.30}): 50 chained sweeps per beta with the
-          per-sweep observables and the final state compared, then one sampled one-step parity after
-          2000 thermalisation sweeps (the sweep is a deterministic function of (theta, seed, t, beta)).
+config 2 (L = 1024, cold, seed 7, beta in {0.90, 1.00, 1.12, 1.30}): 200 chained sweeps per beta with the
+          per-sweep observables and the final state compared, then sampled one-step parities at t = 2000, 5000
+          and 12000 (the sweep is a deterministic function of (theta, seed, t, beta)).
 config 3 (L = 4096, hot, seed 11, PCC beta0 = 1.05, dbeta0 = 1e-3, window 20, target 2/pi): the first 40
           sweeps (two decisions) chained - beta trace and final angles of xy_pcc_run against the oracle's
           controller, and bonds / labels / angles in full at sweeps 0, 10, 20, 30, 39 - then five sampled
-          one-step parities later in the run; the PCC trace at L = 256.
+          one-step parities later in the run; the literal 20 000-sweep schedule at L = 64 and a shortened
+          one at L = 256 with bit-equal beta traces.
 filter    full byte-compare of the bonds of >= 10 sweeps at L = 4096 for beta in {0.5, 1.11996, 5, 50}
           (1.3e9 decisions) against the oracle's fp64 definition: the volume test of the fp32 filter.
 variants  L = 4160 (64-wide tiles with 32-row strips), both label widths; FOURIER at L = 8192.
@@ -72,25 +73,32 @@ def one_step(st, L, seed, beta, where):
 
 
 # ---------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("beta", xy_inputs.CONFIGS[1]["betas"])
-def test_config2_each_beta(xy, beta):
+def test_config2_all_betas(xy):
+    """200 chained sweeps per beta (per-sweep records and final angles), then one-step parities at t = 2000, 5000 and
+    12000 (SURVEY.md:482-485).  The oracle's four chains run side by side on host threads (the C oracle releases the
+    GIL)."""
     cfg = xy_inputs.CONFIGS[1]
-    L, seed, n = cfg["L"], cfg["seed"], 50
+    L, seed, n = cfg["L"], cfg["seed"], 200
     N = L * L
-    st = xy.XYState(L, seed, xy.INIT_COLD)
-    ref = xo.init(L, seed, xo.INIT_COLD)
-    ser_ref = xo.run(ref, L, seed, 0, beta, n)
-    st.sw_sweeps(beta, n)
-    ser = st.get_series(1, n)
-    assert np.array_equal(st.get_angles().view(np.uint32), ref.view(np.uint32)), "angles after 50 chained sweeps"
-    for k in range(n):
+
+    def chain(beta):
+        ref = xo.init(L, seed, xo.INIT_COLD)
+        return ref, xo.run(ref, L, seed, 0, beta, n)
+    with ThreadPoolExecutor(len(cfg["betas"])) as ex:
+        refs = list(ex.map(chain, cfg["betas"]))
+    for beta, (ref, ser_ref) in zip(cfg["betas"], refs):
+        st = xy.XYState(L, seed, xy.INIT_COLD)
+        st.sw_sweeps(beta, n)
+        ser = st.get_series(1, n)
+        assert np.array_equal(st.get_angles().view(np.uint32), ref.view(np.uint32)), f"angles after {n} chained sweeps, beta={beta}"
         for f in OBS_KEYS:
-            assert abs(ser[f][k] - ser_ref[f][k]) <= 1e-9 * N, (beta, k, f)
+            assert np.abs(ser[f] - ser_ref[f]).max() <= 1e-9 * N, (beta, f)
         for f in ("n_bonds_x", "n_bonds_y", "n_clusters", "sweep"):
-            assert ser[f][k] == ser_ref[f][k], (beta, k, f)
-    st.sw_sweeps(beta, cfg["therm"] - n)
-    one_step(st, L, seed, beta, f"cfg2 beta={beta} t={cfg['therm']}")
-    st.destroy()
+            assert np.array_equal(ser[f], ser_ref[f]), (beta, f)
+        for t in (cfg["therm"], 5000, 12000):
+            st.sw_sweeps(beta, t - st.get_sweep())
+            one_step(st, L, seed, beta, f"cfg2 beta={beta} t={t}")
+        st.destroy()
 
 
 def _cfg3_schedules(xy, n, window=None, halve=None):
@@ -140,6 +148,26 @@ def test_config3_first_40_sweeps_chained(xy):
         b.sw_sweeps(beta, more - 1)
         one_step(b, L, seed, beta, f"cfg3 sampled t={b.get_sweep()}")
     b.destroy()
+
+
+def test_config3_literal_schedule_L64(xy):
+    """config 3's schedule as BASELINE.json states it (20 000 sweeps, window 20, dbeta halved every 2000 measured
+    sweeps), chained at L = 64: every beta of the 1000 decisions, beta_mean and the final angles bit for bit"""
+    n = 20000
+    cfg, sg, so = _cfg3_schedules(xy, n)
+    assert (sg.window, sg.halve_every, sg.n_sweeps) == (20, 2000, 20000)
+    L, seed = 64, cfg["seed"]
+    st = xy.XYState(L, seed, xy.INIT_HOT)
+    out = st.pcc_run(cfg["beta0"], sg)
+    ref_theta = xo.init(L, seed, xo.INIT_HOT)
+    ref = xo.pcc_run(ref_theta, L, seed, 0, cfg["beta0"], so, trace_cap=n)
+    assert out["n_decisions"] == ref["n_decisions"] == (n - cfg["discard"]) // cfg["window"]
+    assert np.array_equal(out["trace_beta"], ref["trace_beta"])
+    assert np.abs(out["trace_bY"] - ref["trace_bY"]).max() < 1e-9
+    assert out["beta_final"] == ref["beta_final"] and out["dbeta_final"] == ref["dbeta_final"]
+    assert out["beta_mean"] == ref["beta_mean"]
+    assert np.array_equal(st.get_angles().view(np.uint32), ref_theta.view(np.uint32))
+    st.destroy()
 
 
 def test_config3_pcc_trace_L256(xy):
@@ -234,6 +262,17 @@ def test_fourier_L8192(xy):
     st.sw_sweeps(beta, 1)
     fs = st.get_fourier_series(4, 1)[0]
     assert np.abs(np.concatenate([fs["Fx"], fs["Fy"]]) - F).max() <= 1e-9 * N
+    st.destroy()
+
+
+def test_obs_none_L8192_one_step(xy):
+    """k_bonds<4, 32, bonds, no observables> (fp32 only, two CTAs of 8 warps per SM): the variant every lattice above
+    4096 takes under XY_OBS_NONE, as in bench.py's observables-off legs; one sweep against the oracle in full"""
+    L, seed, beta = 8192, 5, 1.11996
+    st = xy.XYState(L, seed, xy.INIT_HOT)
+    st.set_obs_mode(xy.OBS_NONE)
+    st.sw_sweeps(beta, 3)
+    one_step(st, L, seed, beta, "L=8192 obs off")
     st.destroy()
 
 

@@ -79,6 +79,51 @@ def test_sharded_without_observables(xy):
     _run(xy, 192, 2, seed=8, init="hot", beta=1.12, sweeps=3, obs_none=True)
 
 
+@pytest.mark.parametrize("L,G,init,obs_none", [(8192, 2, "hot", False), (8192, 8, "cold", True), (16384, 4, "hot", False)])
+def test_sharded_large_lattices_take_the_32_row_strip_kernels(xy, L, G, init, obs_none):
+    """L > 4096 selects k_bonds<4, 32, ..., kSlab> (long strips: halo row instead of the y wrap, bond bytes addressed
+    from a base moved back by the slab's offset, whole-lattice Philox counters) and k_flip<4, 32, u32, kSlab> over
+    thousands of tile rows per slab: the regime the paper shards in.  Chained sweeps, everything
+    compared with the whole-lattice oracle (one sweep at L = 16384: an oracle sweep there takes a minute)."""
+    _run(xy, L, G, seed=900 + G, init=init, beta=1.11996, sweeps=2 if L <= 8192 else 1, obs_none=obs_none)
+
+
+def test_hot_slab_is_complete_before_any_exchange(xy):
+    """a hot slab's halo row holds the initial values of the row below it from creation: the partial sums of freshly
+    created slabs (no ShardedLattice, no exchange) add up to the observables of the whole hot lattice"""
+    L, G, seed = 256, 4, 21
+    o = xo.observe(xo.init(L, seed, xo.INIT_HOT), L)
+    slabs = [xy.SlabState(L, L // G, r * (L // G), seed, xy.INIT_HOT) for r in range(G)]
+    part = [s.measure() for s in slabs]
+    for k in ("E", "Mx", "My", "Cx", "Sx", "Cy", "Sy"):
+        assert abs(sum(getattr(p, k) for p in part) - getattr(o, k)) <= 1e-9 * L * L, k
+    for s in slabs:
+        s.destroy()
+
+
+def test_slab_flip_with_a_foreign_record_is_reported_not_written(xy):
+    """rank 0's slab handed the gathered records as if it were rank 1: its edge sites lie outside the slab; the stitch
+    skips them (no out-of-bounds write) and the next blocking call says so; set_angles is refused between the phases"""
+    import torch
+    L, G = 128, 2
+    slabs = [xy.SlabState(L, L // G, r * (L // G), 3, xy.INIT_HOT) for r in range(G)]
+    for s in slabs:
+        s.slab_label(1.12)
+    with pytest.raises(xy.XYError) as e:
+        slabs[0].set_angles(np.zeros(slabs[0].N, np.float32))
+    assert e.value.code == -5
+    gathered = torch.cat([s.edges for s in slabs])
+    slabs[0].slab_flip(gathered, G, 1)                 # wrong rank
+    with pytest.raises(xy.XYError) as e:
+        slabs[0].measure()
+    assert e.value.code == -1 and "outside the slab" in str(e.value)
+    slabs[1].slab_flip(gathered, G, 1)                 # the right one: no complaint
+    slabs[1].measure()
+    slabs[1].get_labels()
+    for s in slabs:
+        s.destroy()
+
+
 def test_slab_errors(xy):
     with pytest.raises(xy.XYError):
         xy.SlabState(128, 48, 0, 1)                 # rows not a multiple of 32
