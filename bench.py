@@ -325,7 +325,7 @@ def run_sharded(args, xy, torch, grp, rank, local_rank, world):
             "config": {"workload": f"{args.workload}: ONE 2D XY lattice L={L} as {world} row slab(s) of {rows} rows, {init} start "
                                    f"seed {seed}, beta={beta}, {therm} thermalisation sweeps untimed",
                        "L": L, "beta": beta, "parallelism": f"row slabs x{world} (shard.py)",
-                       "exchange_bytes_per_sweep_per_rank": {"all_gather_cut_records": 17 * L, "all_gather_first_rows": 4 * L}},
+                       "exchange_bytes_per_sweep_per_rank": {"all_gather_cut_records": 17 * L, "send_recv_first_row": 4 * L}},
             "clocks": clocks, "gpu_launches": int(launches),
             "observables": {"sweep": obs["sweep"], "E_per_site": obs["E"] / N, "m2": (obs["Mx"] ** 2 + obs["My"] ** 2) / N ** 2,
                             "bond_density": (obs["n_bonds_x"] + obs["n_bonds_y"]) / (2 * N), "clusters_per_site": obs["n_clusters"] / N},
@@ -421,6 +421,8 @@ def main():
     ap.add_argument("--beta", type=float, default=None, help="override the workload's beta (sensitivity runs)")
     ap.add_argument("--obs", default="all", choices=["all", "none"],
                     help="none: time the sweeps with the observable sums switched off (xy_set_obs_mode); not the headline")
+    ap.add_argument("--repeats", type=int, default=3,
+                    help="timed runs of K sweeps, each from a re-created state; the median is reported")
     ap.add_argument("--e2e-steps", type=int, default=None)
     ap.add_argument("--shard", action="store_true",
                     help="ONE lattice split into --gpus row slabs (SURVEY 8(f) #3): strong scaling, NCCL all-gather of the "
@@ -462,27 +464,33 @@ def main():
     tw, th = (128, 32) if L % 128 == 0 else (64, 32)
     K, W = args.steps, max(args.warmup, 0)
 
-    st = xy.XYState(L, replica_seed(seed, rank), xy_inputs.INIT_CODE[init], flags=flags)
-    if args.obs == "none":
-        st.set_obs_mode(xy.OBS_NONE)
-    if therm:
-        st.sw_sweeps(beta, therm)
-    st.sw_sweeps(beta, W)
-    torch.cuda.synchronize()
-
-    # ---- timed region 1: K sweeps, configuration resident in HBM ----
+    # ---- timed region 1: K sweeps, configuration resident in HBM; --repeats runs, each from a re-created state
+    #      (same seed, thermalisation and warm-up: the trajectory is deterministic, only the machine varies), the
+    #      MEDIAN run is the reported one (SURVEY.md 8(d) timing protocol) ----
     sampler = ClockSampler(local_rank)
     sampler.start()
-    launches0 = st.get_launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record()
-    st.sw_sweeps(beta, K)
-    e1.record()
-    barrier()
-    ms = max_over_ranks(e0.elapsed_time(e1))
-    launches = st.get_launch_count() - launches0
+    runs, st = [], None
+    for rep in range(max(args.repeats, 1)):
+        if st is not None:
+            st.destroy()
+            st = None
+        st = xy.XYState(L, replica_seed(seed, rank), xy_inputs.INIT_CODE[init], flags=flags)
+        if args.obs == "none":
+            st.set_obs_mode(xy.OBS_NONE)
+        if therm:
+            st.sw_sweeps(beta, therm)
+        st.sw_sweeps(beta, W)
+        torch.cuda.synchronize()
+        launches0 = st.get_launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        st.sw_sweeps(beta, K)
+        e1.record()
+        barrier()
+        runs.append((max_over_ranks(e0.elapsed_time(e1)), st.get_launch_count() - launches0))
     clocks = sampler.stop()
+    ms, launches = sorted(runs)[len(runs) // 2]
     value = whole_job_value(world, N, K, ms)
     obs = st.measure()
 
@@ -591,7 +599,10 @@ def main():
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms / K, "repeats": {"n": len(runs), "ms_per_step": [r[0] / K for r in runs],
+                                               "min": min(r[0] for r in runs) / K, "max": max(r[0] for r in runs) / K,
+                                               "reported": "median"},
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"BASELINE config {cfg_idx + 1 if cfg_idx is not None else '-'} ({args.workload}): "
                                    f"2D XY L={L} periodic, {init} start seed {seed}, beta={beta}, "
