@@ -15,6 +15,7 @@
 #include <limits>
 #include <mutex>
 #include <new>
+#include <utility>
 #include <vector>
 
 using namespace xy;
@@ -75,6 +76,36 @@ Layout make_layout(uint32_t L, uint32_t flags, uint32_t rows = 0, bool slab = fa
     return o;
 }
 
+// The four kernels of a sweep are launched with programmatic stream serialization (xy_device.cuh, pdl_wait): the next
+// kernel's CTAs may become resident and run their prologue while the previous grid drains.  XY_NO_PDL=1 in the
+// environment launches them the plain way, XY_PDL_MASK=<bits> only the named kernels with the attribute (A/B runs).
+enum { PDL_BONDS = 1, PDL_LABEL = 2, PDL_MERGE = 4, PDL_FLIP = 8 };
+int pdl_mask()
+{
+    static const int mask = [] {
+        if (const char *e = getenv("XY_NO_PDL")) if (e[0] == '1') return 0;
+        if (const char *e = getenv("XY_PDL_MASK")) return atoi(e) & 15;
+        return 15;
+    }();
+    return mask;
+}
+
+template <typename... KArgs, typename... Args>
+cudaError_t launch_chain(int which, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args &&...args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = (pdl_mask() & which) ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
+}
+
 // One set of launchers per (tile geometry, label width).
 struct Kernels {
     // what: 0 = sweep with observables, 1 = observables only, 2 = sweep without observables
@@ -96,14 +127,12 @@ struct KS {
     template <bool kB, bool kO, bool kF>
     static cudaError_t bonds_launch(const SweepArgs &a, int grid, cudaStream_t st)
     {
-        k_bonds<VEC, RS, kB, kO, kF><<<grid, BondsShape<kO>::warps * 32, k_bonds_smem_bytes<kO>(), st>>>(a);
-        return cudaGetLastError();
+        return launch_chain(PDL_BONDS, k_bonds<VEC, RS, kB, kO, kF>, grid, BondsShape<kO>::warps * 32, k_bonds_smem_bytes<kO>(), st, a);
     }
     template <bool kB, bool kO>
     static cudaError_t bonds_slab_launch(const SweepArgs &a, int grid, cudaStream_t st)
     {
-        k_bonds<VEC, RS, kB, kO, false, true><<<grid, BondsShape<kO>::warps * 32, k_bonds_smem_bytes<kO>(), st>>>(a);
-        return cudaGetLastError();
+        return launch_chain(PDL_BONDS, k_bonds<VEC, RS, kB, kO, false, true>, grid, BondsShape<kO>::warps * 32, k_bonds_smem_bytes<kO>(), st, a);
     }
     static cudaError_t bonds(const SweepArgs &a, int what, bool fourier, int grid, cudaStream_t st)
     {
@@ -117,23 +146,24 @@ struct KS {
     }
     static void label(const SweepArgs &a, cudaStream_t st)
     {
-        k_label<VEC, R * NW, LabelT><<<a.ntiles, VEC * R * NW, k_label_smem_bytes<VEC, R * NW>(), st>>>(a);
+        launch_chain(PDL_LABEL, k_label<VEC, R * NW, LabelT>, a.ntiles, VEC * R * NW, k_label_smem_bytes<VEC, R * NW>(), st, a);
     }
     static void merge(const SweepArgs &a, cudaStream_t st)
     {
         const uint64_t total = (uint64_t)a.ntiles * (32 * VEC + R * NW);
         uint64_t blocks = (total + 255) / 256;
         if (blocks > 148ull * 64) blocks = 148ull * 64;
-        k_merge<32 * VEC, R * NW, LabelT><<<(unsigned)blocks, 256, 0, st>>>(a);
+        // measured (profiles/r3_pdl.md): above L = 4096 an early-resident k_merge costs more than its launch gap saves
+        launch_chain(a.L <= 4096 ? PDL_MERGE : 0, k_merge<32 * VEC, R * NW, LabelT>, (unsigned)blocks, 256, 0, st, a);
     }
     static void flip(const SweepArgs &a, int grid, cudaStream_t st)
     {
         (void)grid;
-        k_flip<VEC, R * NW, LabelT><<<a.ntiles, VEC * R * NW, 0, st>>>(a);
+        launch_chain(PDL_FLIP, k_flip<VEC, R * NW, LabelT>, a.ntiles, VEC * R * NW, 0, st, a);
     }
     static void flip_slab(const SweepArgs &a, cudaStream_t st)
     {
-        if constexpr (sizeof(LabelT) == 4) k_flip<VEC, R * NW, LabelT, true><<<a.ntiles, VEC * R * NW, 0, st>>>(a);
+        if constexpr (sizeof(LabelT) == 4) launch_chain(PDL_FLIP, k_flip<VEC, R * NW, LabelT, true>, a.ntiles, VEC * R * NW, 0, st, a);
     }
     template <bool kB, bool kO, bool kF>
     static cudaError_t bonds_prepare(int *occ)

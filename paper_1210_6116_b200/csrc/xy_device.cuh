@@ -7,6 +7,15 @@
 
 namespace xy {
 
+// Programmatic dependent launch (sm_90+; cudaLaunchAttributeProgrammaticStreamSerialization): the kernels of a sweep
+// are launched so that the NEXT kernel of the stream may become resident while this grid drains and run its prologue
+// (whatever touches no data of its predecessor).  pdl_wait() returns once the preceding grid has completed and its
+// writes are visible; pdl_launch_next() allows the next grid to be scheduled.  Every kernel calls them in this order,
+// wait first: a grid that could be scheduled before its predecessor passed its own wait could read (in its prologue)
+// data that a kernel two steps back is still writing.  Both are no-ops in a launch without the attribute.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_next() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 constexpr double kTwoPi = 6.283185307179586;   // fl64(2 pi)
 constexpr double kPi    = 3.141592653589793;   // fl64(pi)
 

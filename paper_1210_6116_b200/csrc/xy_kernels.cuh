@@ -302,6 +302,8 @@ k_bonds(const SweepArgs a)
     }
     const uint32_t tab_adj = (uint32_t)__cvta_generic_to_shared(smem_raw)
                              - __float_as_uint(kTabMagic) * BondsEntry<kObs>::bytes;
+    pdl_wait();              // the rotation above reads only the static table: it ran under the previous kernel's tail
+    pdl_launch_next();
     __syncthreads();
 
     // beta: a kernel argument, or (PCC) the controller's; only its two fp32 derivatives stay in registers
@@ -707,6 +709,8 @@ k_label(const SweepArgs a)
     const uint32_t base = r * TW + 32 * w;          // tile-local index of this word's first site
 
     // ---- prep ----
+    pdl_wait();
+    pdl_launch_next();
     uint32_t X, Y;
     {
         const size_t i = (size_t)(y0 + r) * L + x0 + 32 * w;
@@ -862,6 +866,8 @@ template <int TW, int TH, typename LabelT>
 __global__ void __launch_bounds__(256)
 k_merge(const SweepArgs a)
 {
+    pdl_wait();
+    pdl_launch_next();
     const uint32_t L = a.L;
     LabelT *labels = reinterpret_cast<LabelT *>(a.labels);
     const uint64_t total = (uint64_t)a.ntiles * (TW + TH);
@@ -957,6 +963,9 @@ k_flip(const SweepArgs a)
         }
     }
 
+    // theta (final since the previous sweep's k_flip) and the coin rows needed nothing of k_merge
+    pdl_wait();
+    pdl_launch_next();
     // labels are read twice (here and in the last phase; the second read hits L1/L2) rather than
     // held in registers: few registers, so many CTAs per SM hide the latency of the phases
     auto load_labels = [&](size_t i, LabelT (&lab)[4]) {
