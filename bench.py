@@ -535,7 +535,7 @@ def main():
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["achieved_gbs"], "peak": peak,
                 "unit": "GB/s", "frac": kern[dom]["frac"], "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": model[dom] * N,
-                "limited_by": "instruction issue / shared-memory wavefronts, not DRAM (profiles/r2_cfg4.md): the HBM "
+                "limited_by": "instruction issue / shared-memory wavefronts, not DRAM (profiles/r3_cfg4.md): the HBM "
                               "fraction is this kernel's distance from its byte floor",
                 "issue": {"warp_instr_per_launch": imodel.get(dom), "peak_warp_instr_per_s": issue_peak,
                           "frac": kern[dom].get("issue_frac")}}
