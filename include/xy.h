@@ -284,7 +284,8 @@ int xy_slab_label(xy_state *s, double beta, void *cuda_stream);
 /* parity hook: the label phase on an injected bond set of the slab's sites (canonical bytes as xy_get_bonds); the
  * following xy_slab_flip stitches (and flips with the coins of the current sweep counter) */
 int xy_slab_label_bonds(xy_state *s, const uint8_t *host_bonds, size_t n);
-/* dev_gathered_edges: nranks edge records in rank order (device memory) */
+/* dev_gathered_edges: nranks edge records in rank order (device memory).  The table of the replicated union-find is part
+ * of the workspace, sized for L / rows slabs; only a call with another nranks allocates (once) a table of its own. */
 int xy_slab_flip(xy_state *s, const void *dev_gathered_edges, uint32_t nranks, uint32_t rank, void *cuda_stream);
 /* The PCC driver on a sharded lattice (the paper's own use of its multi-GPU code, PAPER.md:62-66 at L >= 8192): the
  * controller (O8) runs replicated on every rank's device, fed with all-reduced sums.  Per measured sweep, after the halo

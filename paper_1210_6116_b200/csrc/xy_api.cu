@@ -48,8 +48,24 @@ constexpr size_t kStageBytes = 64u << 20;  // staging buffer of the debug getter
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-    size_t theta, labels, bonds, rootmask, partials, ring, fring, ctl, tab, edges, xroot, pccbuf, total;
+    size_t theta, labels, bonds, rootmask, partials, ring, fring, ctl, tab, edges, xroot, pccbuf, stitch, total;
 };
+
+// stitch table of a slab for nranks slabs: cap hash slots (key u64 + parent u32) and one slot index per gathered edge entry
+uint32_t stitch_cap(uint64_t entries)
+{
+    uint32_t cap = 1024;
+    while (cap < 4 * entries) cap <<= 1;
+    return cap;
+}
+size_t stitch_bytes(uint32_t L, uint32_t nranks)
+{
+    const uint64_t entries = (uint64_t)nranks * 2u * L;
+    return (size_t)stitch_cap(entries) * 12 + entries * 4;
+}
+// number of equal slabs the lattice splits into when every rank holds `rows` rows: the stitch table inside the workspace is
+// sized for it (another nranks at xy_slab_flip still works: that table is then allocated apart)
+uint32_t default_ranks(uint32_t L, uint32_t rows) { return (L + rows - 1) / rows; }
 
 // rows == L and slab == false: a whole lattice.  A slab holds `rows` rows plus one halo row of
 // theta, its edge record for the all-gather and the table of overridden roots.
@@ -72,6 +88,7 @@ Layout make_layout(uint32_t L, uint32_t flags, uint32_t rows = 0, bool slab = fa
     o.edges = off;    off = align_up(off + (slab ? slab_edge_bytes(L) : 0), 256);
     o.xroot = off;    off = align_up(off + (slab ? (size_t)2 * L * 8 : 0), 256);
     o.pccbuf = off;   off = align_up(off + (slab ? (size_t)16 * 8 : 0), 256);
+    o.stitch = off;   off = align_up(off + (slab ? stitch_bytes(L, default_ranks(L, rows)) : 0), 256);
     o.total = off;
     return o;
 }
@@ -300,8 +317,9 @@ struct xy_state {
     uint32_t rows = 0, y_off = 0;   // the state holds rows [y_off, y_off + rows) of the L x L lattice (rows == L: all of it)
     bool slab = false;              // created by xy_slab_create: open in y, halo row, stitch
     bool slab_labelled = false;     // xy_slab_label done, xy_slab_flip pending
-    StitchTable stitch{};           // replicated union-find over the cut roots (device memory, allocated at the first flip)
-    uint32_t stitch_ranks = 0;
+    StitchTable stitch{};           // replicated union-find over the cut roots: inside the workspace for L / rows slabs,
+    uint32_t stitch_ranks = 0;      //   allocated apart (stitch_owned) if xy_slab_flip is called with another nranks
+    bool stitch_owned = false;
     SweepArgs pending{};            // arguments of the sweep between xy_slab_label and xy_slab_flip
     uint64_t N = 0, seed = 0;       // N: sites held by this state
     uint64_t T = 0;                 // sweeps done
@@ -351,6 +369,16 @@ struct DeviceGuard {
     explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
     ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
+
+void set_stitch(xy_state *s, void *p, uint32_t nranks)
+{
+    const uint32_t cap = stitch_cap((uint64_t)nranks * 2u * s->L);
+    s->stitch.key = static_cast<uint64_t *>(p);
+    s->stitch.parent = reinterpret_cast<uint32_t *>(s->stitch.key + cap);
+    s->stitch.slot_of = s->stitch.parent + cap;
+    s->stitch.cap_mask = cap - 1;
+    s->stitch_ranks = nranks;
+}
 
 int check_L(uint32_t L)
 {
@@ -588,6 +616,7 @@ static int create_common(xy_state **out, uint32_t L, uint32_t rows, uint32_t y_o
         s->ws = static_cast<char *>(p);
         s->owns_ws = true;
     }
+    if (slab) set_stitch(s, s->ws + s->lay.stitch, default_ranks(L, rows));   // no allocation in the sweep loop
     int bo = 0, bn = 0, fl = 0, sms = 0;
     cudaError_t e = (cudaError_t)s->ker.prepare(s->fourier(), &bo, &bn, &fl);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, s->device);
@@ -672,7 +701,7 @@ int xy_destroy(xy_state *s)
     cudaStreamSynchronize(s->stream);
     for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
     if (s->stage) cudaFree(s->stage);
-    if (s->stitch.key) cudaFree(s->stitch.key);
+    if (s->stitch_owned) cudaFree(s->stitch.key);
     if (s->owns_ws) cudaFree(s->ws);
     delete s;
     return XY_OK;
@@ -1343,16 +1372,15 @@ int xy_slab_flip(xy_state *s, const void *dev_gathered_edges, uint32_t nranks, u
     const uint64_t entries = (uint64_t)nranks * 2u * s->L;
     if (entries >= (1ull << 29)) return fail(XY_ERR_ARG, "too many cut sites");
     if (s->stitch_ranks != nranks) {
-        if (s->stitch.key) { CUDA_TRY(cudaStreamSynchronize(s->stream)); cudaFree(s->stitch.key); s->stitch = StitchTable{}; }
-        uint32_t cap = 1024;
-        while (cap < 4 * entries) cap <<= 1;
+        // not the number of slabs the workspace table was sized for (create_common): a table of its own
+        if (s->stitch_owned) { CUDA_TRY(cudaStreamSynchronize(s->stream)); cudaFree(s->stitch.key); }
+        s->stitch = StitchTable{};
+        s->stitch_owned = false;
+        s->stitch_ranks = 0;
         void *p = nullptr;
-        CUDA_TRY(cudaMalloc(&p, (size_t)cap * 12 + entries * 4));
-        s->stitch.key = static_cast<uint64_t *>(p);
-        s->stitch.parent = reinterpret_cast<uint32_t *>(s->stitch.key + cap);
-        s->stitch.slot_of = s->stitch.parent + cap;
-        s->stitch.cap_mask = cap - 1;
-        s->stitch_ranks = nranks;
+        CUDA_TRY(cudaMalloc(&p, stitch_bytes(s->L, nranks)));
+        set_stitch(s, p, nranks);
+        s->stitch_owned = true;
     }
     const unsigned char *gathered = static_cast<const unsigned char *>(dev_gathered_edges);
     const int grid = 148 * 4;

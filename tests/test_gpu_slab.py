@@ -88,6 +88,25 @@ def test_sharded_large_lattices_take_the_32_row_strip_kernels(xy, L, G, init, ob
     _run(xy, L, G, seed=900 + G, init=init, beta=1.11996, sweeps=2 if L <= 8192 else 1, obs_none=obs_none)
 
 
+def test_unequal_slabs(xy):
+    """slabs of 32, 32 and 64 rows: nranks = 3 is not L / rows for any of them, so every rank's stitch table is the
+    separately allocated one (the table inside the workspace is sized for equal slabs); three chained sweeps against
+    the whole-lattice oracle"""
+    from paper_1210_6116_b200 import shard
+    L, seed, beta = 128, 77, 1.12
+    rows, y_off = [32, 32, 64], [0, 32, 64]
+    ref = xo.init(L, seed, xo.INIT_HOT)
+    lats = shard.run_threads(3, lambda r, comm: shard.ShardedLattice(xy.SlabState(L, rows[r], y_off[r], seed, xy.INIT_HOT), comm))
+    for t in range(3):
+        shard.run_threads(3, lambda r, comm: lats[r].sweep(beta))
+        b, lab, o = xo.sweep(ref, L, seed, t, beta)
+        assert (np.concatenate([lat.slab.get_bonds() for lat in lats]) == b).all(), t
+        assert (np.concatenate([lat.slab.get_labels() for lat in lats]) == lab).all(), t
+        assert (np.concatenate([lat.slab.get_angles() for lat in lats]) == ref).all(), t
+    for lat in lats:
+        lat.slab.destroy()
+
+
 def test_hot_slab_is_complete_before_any_exchange(xy):
     """a hot slab's halo row holds the initial values of the row below it from creation: the partial sums of freshly
     created slabs (no ShardedLattice, no exchange) add up to the observables of the whole hot lattice"""
